@@ -1,0 +1,159 @@
+/* rick_b200.h -- C ABI of librick_b200: the single-GPU w-stacking imaging hot path on NVIDIA B200 (sm_100a).
+ *
+ * What it computes (citations: P:n = PAPER.md line n of arXiv 2411.07321; D1-D9 = the readings listed
+ * in DESIGN.md "Readings of the paper"):
+ *
+ *   rick_bin                   per-visibility nearest cell / nearest w-plane / keep-drop decision and a
+ *                              stable device radix sort by (w-plane, 32x32 uv tile) key.  Replaces the
+ *                              paper's per-slab bucket arrays; "visibilities are mapped to the
+ *                              closest w-plane".                                     [D2-D5]
+ *   rick_grid                  convolutional gridding, Eq. 3, with the separable truncated
+ *                              Gaussian G = g(i-x) g(j-y), g(d) = exp(-d^2 / 2 sigma^2).         [D6]
+ *   rick_fft_planes            un-normalised inverse 2-D DFT (sign +) of every w-plane,
+ *                              batched cuFFT C2C / Z2Z, in place.                                [D7]
+ *   rick_wcorrect_accumulate   phase screen exp(+2 pi i w_k (sqrt(1-l^2-m^2)-1)), sum over planes
+ *                              (Eq. 2; step 4) and division by the kernel taper.     [D8]
+ *   rick_image                 hands the fp64 N x N dirty image to the caller.
+ *
+ * Conventions
+ *   - Every function returns RICK_OK (0) or a negative rick_status; nothing throws or exits.
+ *   - "device" pointers are CUDA device pointers on the current device, "host" pointers are host memory.
+ *     The caller owns every buffer it passes; the library owns only the plan (geometry constants, the
+ *     1-D taper table, the cuFFT handle, stage-timing events).  No allocation happens after
+ *     rick_plan_create / rick_plan_set_dtype.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
+ *     enqueued asynchronously on it unless stated otherwise.
+ *   - Geometry [D1]: du = 1/(N dl).  Mesh node i <-> u = (i - N/2) du; pixel p <-> l = (p - N/2) dl.
+ *   - Layouts: mesh grid[k][j][i], i (u) fastest, interleaved (re, im), float2 (RICK_C64) or double2
+ *     (RICK_C128); image[q][p], p (l) fastest, q <-> m, fp64.
+ *   - Modulated mesh: rick_grid stores (-1)^(i+j) * V~(u_i, v_j, w_k) and rick_wcorrect_accumulate
+ *     applies (-1)^(p+q); with the plain (un-shifted) cuFFT in between this equals the centred
+ *     transform of D7 exactly (sign flips only, N even).  A caller comparing the mesh with Eq. 3 must
+ *     multiply by the checkerboard.
+ *   - Precision: RICK_C64 keeps visibility x weight x taps, the mesh and the FFT in fp32;
+ *     coordinates, indices, the fractional offsets (before narrowing), the w phase, the plane sum and
+ *     the image are fp64.  RICK_C128 is fp64 throughout.
+ */
+#ifndef RICK_B200_H
+#define RICK_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rick_plan rick_plan; /* opaque */
+
+typedef enum {
+    RICK_OK = 0,
+    RICK_EINVAL = -1,  /* bad argument (see each function) */
+    RICK_ENOMEM = -2,  /* a caller-provided workspace is too small, or plan allocation failed */
+    RICK_ECUDA = -3,   /* a CUDA runtime call or kernel launch failed */
+    RICK_ECUFFT = -4,  /* a cuFFT call failed */
+    RICK_ESTATE = -5   /* call order: rick_grid before rick_bin, FFT before rick_plan_set_dtype, ... */
+} rick_status;
+
+typedef enum { RICK_C64 = 0, RICK_C128 = 1 } rick_dtype;
+
+/* stage indices of rick_get_timings */
+enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_WCORRECT = 4,
+       RICK_T_IMAGE = 5, RICK_T_COUNT = 6 };
+
+/* Create a plan (BASELINE.json north_star (1)).  Host-synchronous.
+ *   N        mesh and image size per axis; a multiple of 32 (tile size), 32 <= N <= 32768
+ *   Nw       number of w-planes, 1 <= Nw <= 4096, Nw (N/32)^2 < 2^31
+ *   support  full footprint width S in cells, odd, 3 <= S <= 15  (h = (S-1)/2)
+ *   sigma    Gaussian width in cells, > 0
+ *   w_min, w_max   w range covered by the Nw planes, w_max > w_min; plane k is centred at
+ *            w_min + (k + 1/2)(w_max - w_min)/Nw  [D3]
+ *   dl       pixel size (direction cosine per pixel), > 0, N dl < sqrt(2)
+ * Errors: RICK_EINVAL, RICK_ENOMEM, RICK_ECUDA.  The mesh dtype defaults to RICK_C64. */
+int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, double w_max, double dl,
+                     rick_plan** out);
+
+/* Select the mesh dtype and (re)build the cuFFT plan for it.  Host-synchronous. */
+int rick_plan_set_dtype(rick_plan* plan, int dtype);
+
+/* Sizes of the two caller-provided scratch buffers: `bin_bytes` for rick_bin with up to M
+ * visibilities, `fft_bytes` for rick_fft_planes (0 if cuFFT needs none).  Either pointer may be NULL. */
+int rick_plan_workspace_bytes(const rick_plan* plan, long long M, size_t* bin_bytes, size_t* fft_bytes);
+
+int rick_plan_destroy(rick_plan* plan);
+
+/* Key generation + stable radix sort + gather.  [D2-D5], BASELINE.json north_star (2).
+ *   M                     number of visibilities, 0 <= M < 2^32 - 1
+ *   u, v, w               device float[M], baseline coordinates in wavelengths
+ *   vis                   device float2[M] (complex64), weight: device float[M]
+ *   u_s .. weight_s       device outputs of capacity M: the kept visibilities in the stable order
+ *                         (key, input index); only the first n_kept entries are written
+ *   key_out               nullable device unsigned[M]: key of every input visibility,
+ *                         key = (k T + (j0 >> 5)) T + (i0 >> 5), T = N/32; dropped -> Nw T^2
+ *   perm_out              nullable device unsigned[M]: sorted rank -> input index (all M, sentinels last)
+ *   bin_start_out         nullable device unsigned long long[Nw T^2 + 2]: number of visibilities with
+ *                         key < b (entry Nw T^2 is n_kept, the last entry is M)
+ *   workspace             device scratch of at least rick_plan_workspace_bytes(M) bytes, 256-byte aligned
+ *   n_kept_dev            device long long: number of kept visibilities
+ * A visibility is dropped whole (never clipped or wrapped) when any of its six numbers is non-finite,
+ * its footprint would leave the mesh, or w lies outside [w_min, w_max]  [D5]; that is not an error.
+ * The sorted arrays, n_kept_dev and the workspace are bound to the plan and must stay valid and
+ * unmodified until the last rick_grid call that uses them.
+ * Errors: RICK_EINVAL (null pointer, M out of range), RICK_ENOMEM (workspace too small), RICK_ECUDA. */
+int rick_bin(rick_plan* plan, long long M, const float* u, const float* v, const float* w,
+             const void* vis, const float* weight, float* u_s, float* v_s, float* w_s, void* vis_s,
+             float* weight_s, unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out,
+             void* workspace, size_t workspace_bytes, long long* n_kept_dev, void* stream);
+
+/* Gridding, Eq. 3 [D6], of the visibilities bound by the last rick_bin into
+ * grid[Nw][N][N] (device, dtype of the plan, caller-owned).  zero_first != 0 clears the mesh first;
+ * zero_first == 0 accumulates onto its contents (chunked inputs).
+ * Errors: RICK_ESTATE (no rick_bin yet), RICK_EINVAL, RICK_ECUDA. */
+int rick_grid(rick_plan* plan, void* grid, int zero_first, void* stream);
+
+/* In-place un-normalised inverse 2-D DFT of every plane [D7].  fft_work: device scratch of at least
+ * the `fft_bytes` reported by rick_plan_workspace_bytes (may be NULL when that is 0).
+ * Errors: RICK_ESTATE (dtype never set), RICK_ENOMEM, RICK_ECUFFT. */
+int rick_fft_planes(rick_plan* plan, void* grid, void* fft_work, size_t fft_work_bytes, void* stream);
+
+/* image[q][p] (+)= (1 / (t[p] t[q])) sum_k Re{ exp(+2 pi i w_k nm1(q,p)) P_k[q][p] },
+ * nm1 = -(l^2+m^2)/(1+sqrt(1-l^2-m^2)), t = 1-D taper of the truncated Gaussian [D8].
+ * Reads every transformed plane once.  image: device double[N*N]. */
+int rick_wcorrect_accumulate(rick_plan* plan, const void* grid, double* image, int zero_first,
+                             void* stream);
+
+/* Copy the fp64 image to `out` (device if out_is_host == 0, host otherwise; asynchronous either way:
+ * synchronise the stream before reading a host buffer). */
+int rick_image(rick_plan* plan, const double* image_dev, double* out, int out_is_host, void* stream);
+
+/* Device buffers for rick_image_from_host (all caller-owned, capacity M where per-visibility). */
+typedef struct {
+    float *u, *v, *w; void* vis; float* weight;          /* staging for the inputs */
+    float *u_s, *v_s, *w_s; void* vis_s; float* weight_s;/* sorted copies */
+    void* workspace; size_t workspace_bytes;             /* rick_bin scratch */
+    void* grid;                                          /* Nw*N*N complex mesh */
+    void* fft_work; size_t fft_work_bytes;
+    double* image;                                       /* N*N */
+    long long* n_kept;                                   /* device scalar */
+} rick_device_buffers;
+
+/* The whole path from HOST buffers to a HOST image: H2D copies of the five input arrays, rick_bin,
+ * rick_grid (zero_first), rick_fft_planes, rick_wcorrect_accumulate (zero_first), D2H of the image.
+ * Everything is enqueued on `stream`; the call returns after synchronising it.  Host buffers should
+ * be pinned for the copies to run at full speed. */
+int rick_image_from_host(rick_plan* plan, long long M, const float* u_host, const float* v_host,
+                         const float* w_host, const void* vis_host, const float* weight_host,
+                         const rick_device_buffers* dev, double* image_host, void* stream);
+
+/* CUDA-event times (milliseconds) of the most recent call of each stage, indexed by RICK_T_*;
+ * stages never run report 0.  Synchronises on the recorded events.  n <= RICK_T_COUNT. */
+int rick_get_timings(rick_plan* plan, double* ms, int n);
+
+/* Number of kernel launches (library kernels + cuFFT exec calls) issued through this plan so far. */
+long long rick_launch_count(const rick_plan* plan);
+
+const char* rick_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RICK_B200_H */

@@ -1,0 +1,285 @@
+"""Thin ctypes binding of librick_b200 (include/rick_b200.h): argument marshalling only.
+
+PyTorch owns device memory and streams; every step of the hot path runs inside the library's CUDA
+kernels (plus batched cuFFT for the plane transforms).  There is no CPU fallback: if the shared library
+is missing or cannot be loaded, importing symbols from it raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import torch
+
+from . import build as _build
+
+RICK_C64, RICK_C128 = 0, 1
+RICK_T_NAMES = ("bin", "zero", "grid", "fft", "wcorrect", "image")
+
+_lib = None
+
+EXPORTS = (
+    "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
+    "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
+    "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
+)
+
+
+class RickError(RuntimeError):
+    pass
+
+
+class _DeviceBuffers(C.Structure):
+    _fields_ = [
+        ("u", C.c_void_p), ("v", C.c_void_p), ("w", C.c_void_p), ("vis", C.c_void_p), ("weight", C.c_void_p),
+        ("u_s", C.c_void_p), ("v_s", C.c_void_p), ("w_s", C.c_void_p), ("vis_s", C.c_void_p), ("weight_s", C.c_void_p),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+        ("grid", C.c_void_p),
+        ("fft_work", C.c_void_p), ("fft_work_bytes", C.c_size_t),
+        ("image", C.c_void_p),
+        ("n_kept", C.c_void_p),
+    ]
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load librick_b200.so (built in-tree by __graft_entry__.build()); fails loudly when absent."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise RickError(f"{path} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                            "(the CUDA library is the only implementation; there is no fallback)")
+        L = C.CDLL(path)
+        vp, ll, sz, dbl, i = C.c_void_p, C.c_longlong, C.c_size_t, C.c_double, C.c_int
+        L.rick_plan_create.argtypes = [i, i, i, dbl, dbl, dbl, dbl, C.POINTER(vp)]
+        L.rick_plan_set_dtype.argtypes = [vp, i]
+        L.rick_plan_workspace_bytes.argtypes = [vp, ll, C.POINTER(sz), C.POINTER(sz)]
+        L.rick_plan_destroy.argtypes = [vp]
+        L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
+        L.rick_grid.argtypes = [vp, vp, i, vp]
+        L.rick_fft_planes.argtypes = [vp, vp, vp, sz, vp]
+        L.rick_wcorrect_accumulate.argtypes = [vp, vp, vp, i, vp]
+        L.rick_image.argtypes = [vp, vp, vp, i, vp]
+        L.rick_image_from_host.argtypes = [vp, ll, vp, vp, vp, vp, vp, C.POINTER(_DeviceBuffers), vp, vp]
+        L.rick_get_timings.argtypes = [vp, C.POINTER(dbl), i]
+        L.rick_launch_count.argtypes = [vp]
+        L.rick_launch_count.restype = ll
+        L.rick_strerror.argtypes = [i]
+        L.rick_strerror.restype = C.c_char_p
+        for name in EXPORTS:
+            getattr(L, name)
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise RickError(f"{what} failed: {lib().rick_strerror(rc).decode()} ({rc})")
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream=None) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return s.cuda_stream
+
+
+def _dev(t: torch.Tensor, dtype, n: Optional[int] = None, what: str = "tensor") -> torch.Tensor:
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise RickError(f"{what}: expected a contiguous CUDA tensor of {dtype}")
+    if n is not None and t.numel() < n:
+        raise RickError(f"{what}: needs at least {n} elements")
+    return t
+
+
+# ---- the C entry points, one Python function each ---------------------------------------------
+
+def rick_plan_create(N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float) -> int:
+    h = C.c_void_p()
+    _check(lib().rick_plan_create(N, Nw, support, sigma, w_min, w_max, dl, C.byref(h)), "rick_plan_create")
+    return h.value
+
+
+def rick_plan_set_dtype(plan: int, dtype: int) -> None:
+    _check(lib().rick_plan_set_dtype(plan, dtype), "rick_plan_set_dtype")
+
+
+def rick_plan_workspace_bytes(plan: int, M: int):
+    a, b = C.c_size_t(), C.c_size_t()
+    _check(lib().rick_plan_workspace_bytes(plan, M, C.byref(a), C.byref(b)), "rick_plan_workspace_bytes")
+    return int(a.value), int(b.value)
+
+
+def rick_plan_destroy(plan: int) -> None:
+    _check(lib().rick_plan_destroy(plan), "rick_plan_destroy")
+
+
+def rick_bin(plan: int, M: int, u, v, w, vis, weight, u_s, v_s, w_s, vis_s, weight_s, workspace, n_kept,
+             key_out=None, perm_out=None, bin_start_out=None, stream=None) -> None:
+    f32, c64 = torch.float32, torch.complex64
+    for t, dt, nm in ((u, f32, "u"), (v, f32, "v"), (w, f32, "w"), (vis, c64, "vis"), (weight, f32, "weight"),
+                      (u_s, f32, "u_s"), (v_s, f32, "v_s"), (w_s, f32, "w_s"), (vis_s, c64, "vis_s"),
+                      (weight_s, f32, "weight_s")):
+        _dev(t, dt, M, nm)
+    _dev(workspace, torch.uint8, None, "workspace")
+    _dev(n_kept, torch.int64, 1, "n_kept")
+    if key_out is not None:
+        _dev(key_out, torch.int32, M, "key_out")
+    if perm_out is not None:
+        _dev(perm_out, torch.int32, M, "perm_out")
+    if bin_start_out is not None:
+        _dev(bin_start_out, torch.int64, None, "bin_start_out")
+    _check(lib().rick_bin(plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight), _ptr(u_s), _ptr(v_s),
+                          _ptr(w_s), _ptr(vis_s), _ptr(weight_s), _ptr(key_out), _ptr(perm_out),
+                          _ptr(bin_start_out), _ptr(workspace), workspace.numel(), _ptr(n_kept), _stream(stream)),
+           "rick_bin")
+
+
+def rick_grid(plan: int, grid: torch.Tensor, zero_first: bool = True, stream=None) -> None:
+    if not (grid.is_cuda and grid.is_contiguous()):
+        raise RickError("grid: expected a contiguous CUDA tensor")
+    _check(lib().rick_grid(plan, _ptr(grid), 1 if zero_first else 0, _stream(stream)), "rick_grid")
+
+
+def rick_fft_planes(plan: int, grid: torch.Tensor, fft_work: Optional[torch.Tensor], stream=None) -> None:
+    nbytes = 0 if fft_work is None else fft_work.numel() * fft_work.element_size()
+    _check(lib().rick_fft_planes(plan, _ptr(grid), _ptr(fft_work), nbytes, _stream(stream)), "rick_fft_planes")
+
+
+def rick_wcorrect_accumulate(plan: int, grid: torch.Tensor, image: torch.Tensor, zero_first: bool = True,
+                             stream=None) -> None:
+    _dev(image, torch.float64, None, "image")
+    _check(lib().rick_wcorrect_accumulate(plan, _ptr(grid), _ptr(image), 1 if zero_first else 0, _stream(stream)),
+           "rick_wcorrect_accumulate")
+
+
+def rick_image(plan: int, image_dev: torch.Tensor, out: torch.Tensor, stream=None) -> None:
+    _dev(image_dev, torch.float64, None, "image_dev")
+    if out.dtype != torch.float64 or not out.is_contiguous() or out.numel() < image_dev.numel():
+        raise RickError("out: expected a contiguous float64 tensor of N*N elements")
+    _check(lib().rick_image(plan, _ptr(image_dev), _ptr(out), 0 if out.is_cuda else 1, _stream(stream)), "rick_image")
+
+
+def rick_get_timings(plan: int) -> Dict[str, float]:
+    arr = (C.c_double * len(RICK_T_NAMES))()
+    _check(lib().rick_get_timings(plan, arr, len(RICK_T_NAMES)), "rick_get_timings")
+    return {n: float(arr[i]) for i, n in enumerate(RICK_T_NAMES)}
+
+
+def rick_launch_count(plan: int) -> int:
+    return int(lib().rick_launch_count(plan))
+
+
+# ---- buffer ownership helper (allocation + marshalling; no arithmetic) --------------------------
+
+class Imager:
+    """Owns the plan handle and the torch device buffers for one configuration and calls the C entry
+    points in path order.  Nothing is computed in Python."""
+
+    def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
+                 dtype: str = "c64", M_max: int = 0, device="cuda"):
+        if not torch.cuda.is_available():
+            raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
+        self.device = torch.device(device)
+        self.N, self.Nw, self.support = N, Nw, support
+        self.dtype = RICK_C128 if dtype == "c128" else RICK_C64
+        self.cdtype = torch.complex128 if dtype == "c128" else torch.complex64
+        with torch.cuda.device(self.device):
+            self.plan = rick_plan_create(N, Nw, support, sigma, w_min, w_max, dl)
+            rick_plan_set_dtype(self.plan, self.dtype)
+        self.M_max = 0
+        self.grid = torch.empty((Nw, N, N), dtype=self.cdtype, device=self.device)
+        self.image = torch.empty((N, N), dtype=torch.float64, device=self.device)
+        self.n_kept = torch.zeros(1, dtype=torch.int64, device=self.device)
+        _, fft_bytes = rick_plan_workspace_bytes(self.plan, 0)
+        self.fft_work = torch.empty(fft_bytes, dtype=torch.uint8, device=self.device) if fft_bytes else None
+        self.sorted = None
+        self.workspace = None
+        self.staging = None
+        self.reserve(M_max)
+
+    def reserve(self, M: int) -> None:
+        if M <= self.M_max and self.sorted is not None:
+            return
+        m = max(int(M), 1)
+        d = self.device
+        self.sorted = dict(u=torch.empty(m, dtype=torch.float32, device=d), v=torch.empty(m, dtype=torch.float32, device=d),
+                           w=torch.empty(m, dtype=torch.float32, device=d), vis=torch.empty(m, dtype=torch.complex64, device=d),
+                           weight=torch.empty(m, dtype=torch.float32, device=d))
+        bin_bytes, _ = rick_plan_workspace_bytes(self.plan, m)
+        self.workspace = torch.empty(bin_bytes, dtype=torch.uint8, device=d)
+        self.staging = None
+        self.M_max = m
+
+    def close(self) -> None:
+        if self.plan:
+            rick_plan_destroy(self.plan)
+            self.plan = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # path steps
+    def bin(self, u, v, w, vis, weight, key_out=None, perm_out=None, bin_start_out=None) -> None:
+        M = int(u.numel())
+        self.reserve(M)
+        s = self.sorted
+        rick_bin(self.plan, M, u, v, w, vis, weight, s["u"], s["v"], s["w"], s["vis"], s["weight"], self.workspace,
+                 self.n_kept, key_out=key_out, perm_out=perm_out, bin_start_out=bin_start_out)
+
+    def grid_(self, zero_first: bool = True) -> None:
+        rick_grid(self.plan, self.grid, zero_first)
+
+    def fft(self) -> None:
+        rick_fft_planes(self.plan, self.grid, self.fft_work)
+
+    def wcorrect(self, zero_first: bool = True) -> None:
+        rick_wcorrect_accumulate(self.plan, self.grid, self.image, zero_first)
+
+    def run(self, u, v, w, vis, weight) -> torch.Tensor:
+        """bin -> grid -> FFT -> w-correct on device-resident inputs; returns the device image."""
+        self.bin(u, v, w, vis, weight)
+        self.grid_(True)
+        self.fft()
+        self.wcorrect(True)
+        return self.image
+
+    def run_from_host(self, u, v, w, vis, weight, image_host: torch.Tensor) -> torch.Tensor:
+        """rick_image_from_host: host (pinned) inputs -> host image, copies included."""
+        M = int(u.numel())
+        self.reserve(M)
+        if self.staging is None:
+            d = self.device
+            m = self.M_max
+            self.staging = dict(u=torch.empty(m, dtype=torch.float32, device=d), v=torch.empty(m, dtype=torch.float32, device=d),
+                                w=torch.empty(m, dtype=torch.float32, device=d), vis=torch.empty(m, dtype=torch.complex64, device=d),
+                                weight=torch.empty(m, dtype=torch.float32, device=d))
+        for t in (u, v, w, vis, weight, image_host):
+            if t.is_cuda or not t.is_contiguous():
+                raise RickError("run_from_host: host tensors expected")
+        g, s = self.staging, self.sorted
+        b = _DeviceBuffers(
+            _ptr(g["u"]), _ptr(g["v"]), _ptr(g["w"]), _ptr(g["vis"]), _ptr(g["weight"]),
+            _ptr(s["u"]), _ptr(s["v"]), _ptr(s["w"]), _ptr(s["vis"]), _ptr(s["weight"]),
+            _ptr(self.workspace), self.workspace.numel(), _ptr(self.grid),
+            _ptr(self.fft_work), 0 if self.fft_work is None else self.fft_work.numel(),
+            _ptr(self.image), _ptr(self.n_kept))
+        _check(lib().rick_image_from_host(self.plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight),
+                                          C.byref(b), _ptr(image_host), _stream()), "rick_image_from_host")
+        return image_host
+
+    def timings(self) -> Dict[str, float]:
+        return rick_get_timings(self.plan)
+
+    def launches(self) -> int:
+        return rick_launch_count(self.plan)

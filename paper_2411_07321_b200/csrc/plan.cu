@@ -1,0 +1,302 @@
+// plan.cu -- plan lifetime, cuFFT stage, stage timers, host<->device entry points of librick_b200.
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "rick_internal.cuh"
+
+namespace {
+
+int ceil_log2_u64(unsigned long long v) {   // smallest b with 2^b > v  (bits needed to store v)
+    int b = 0;
+    while (b < 63 && (1ull << b) <= v) ++b;
+    return b;
+}
+
+struct StageTimer {
+    rick_plan* p;
+    int stage;
+    cudaStream_t st;
+    StageTimer(rick_plan* p_, int s_, cudaStream_t st_) : p(p_), stage(s_), st(st_) {
+        cudaEventRecord(p->ev_start[stage], st);
+    }
+    ~StageTimer() {
+        cudaEventRecord(p->ev_stop[stage], st);
+        p->ev_valid[stage] = true;
+    }
+};
+
+void destroy_fft(rick_plan* p) {
+    if (p->fft_ready) {
+        cufftDestroy(p->fft);
+        p->fft_ready = false;
+    }
+}
+
+// Largest batch (a divisor of Nw) whose cuFFT work area stays within `limit` bytes.
+int build_fft(rick_plan* p) {
+    destroy_fft(p);
+    const long long N = p->g.N;
+    const cufftType type = (p->dtype == RICK_C128) ? CUFFT_Z2Z : CUFFT_C2C;
+    const size_t limit = (size_t)8 << 30;
+    for (int batch = p->g.Nw; batch >= 1; --batch) {
+        if (p->g.Nw % batch) continue;
+        cufftHandle h;
+        if (cufftCreate(&h) != CUFFT_SUCCESS) return RICK_ECUFFT;
+        if (cufftSetAutoAllocation(h, 0) != CUFFT_SUCCESS) { cufftDestroy(h); return RICK_ECUFFT; }
+        long long n[2] = {N, N};
+        size_t work = 0;
+        cufftResult r = cufftMakePlanMany64(h, 2, n, NULL, 1, N * N, NULL, 1, N * N, type, batch, &work);
+        if (r != CUFFT_SUCCESS) {
+            cufftDestroy(h);
+            if (batch == 1) return RICK_ECUFFT;
+            continue;
+        }
+        if (work > limit && batch > 1) {
+            cufftDestroy(h);
+            continue;
+        }
+        p->fft = h;
+        p->fft_ready = true;
+        p->fft_batch = batch;
+        p->fft_work_bytes = work;
+        return RICK_OK;
+    }
+    return RICK_ECUFFT;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, double w_max, double dl,
+                     rick_plan** out) {
+    if (!out) return RICK_EINVAL;
+    *out = NULL;
+    if (N < 32 || N > 32768 || (N % RICK_TILE) != 0) return RICK_EINVAL;
+    if (Nw < 1 || Nw > 4096) return RICK_EINVAL;
+    if (support < 3 || support > 15 || (support % 2) == 0) return RICK_EINVAL;
+    if (!(sigma > 0.0) || !isfinite(sigma)) return RICK_EINVAL;
+    if (!isfinite(w_min) || !isfinite(w_max) || !(w_max > w_min)) return RICK_EINVAL;
+    if (!(dl > 0.0) || !isfinite(dl) || !((double)N * dl < 1.4142135623730951)) return RICK_EINVAL;
+    const long long T = N / RICK_TILE;
+    const long long n_bins = (long long)Nw * T * T;
+    if (n_bins >= (1ll << 31)) return RICK_EINVAL;
+
+    rick_plan* p = new (std::nothrow) rick_plan();
+    if (!p) return RICK_ENOMEM;
+    memset(p, 0, sizeof(*p));
+    RickGeom& g = p->g;
+    g.N = N; g.Nw = Nw; g.S = support; g.h = (support - 1) / 2; g.T = (int)T;
+    g.s = (double)N * dl;
+    g.half = (double)(N / 2);
+    g.w_min = w_min; g.w_max = w_max;
+    g.inv_dw = (double)Nw / (w_max - w_min);
+    g.dl = dl;
+    g.dw = (w_max - w_min) / (double)Nw;
+    g.sigma = sigma;
+    g.n_bins = (uint32_t)n_bins;
+    p->dtype = RICK_C64;
+
+    // radix-sort digit layout: keys take values 0 .. n_bins (the sentinel), LSD passes of <= 8 bits
+    p->key_bits = ceil_log2_u64((unsigned long long)n_bins);
+    if (p->key_bits < 1) p->key_bits = 1;
+    p->n_pass = (p->key_bits + RICK_RADIX_BITS_MAX - 1) / RICK_RADIX_BITS_MAX;
+    {
+        int shift = 0;
+        for (int i = 0; i < p->n_pass; ++i) {
+            int bits = p->key_bits / p->n_pass + (i < (p->key_bits % p->n_pass) ? 1 : 0);
+            p->digit_bits[i] = bits;
+            p->digit_shift[i] = shift;
+            shift += bits;
+        }
+    }
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { delete p; return RICK_ECUDA; }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { delete p; return RICK_ECUDA; }
+    p->sm_count = sms > 0 ? sms : 148;
+
+    // D8 1-D taper: t[p] = c0 exp(-2 pi^2 sigma^2 nu_p^2), c0 = sigma sqrt(2 pi) erf((h + 1/2)/(sigma sqrt 2))
+    double* inv_t = (double*)malloc(sizeof(double) * (size_t)N);
+    if (!inv_t) { delete p; return RICK_ENOMEM; }
+    {
+        const double pi = 3.14159265358979323846;
+        const double a_t = (double)g.h + 0.5;
+        const double c0 = sigma * sqrt(2.0 * pi) * erf(a_t / (sigma * sqrt(2.0)));
+        for (int i = 0; i < N; ++i) {
+            const double nu = (double)(i - N / 2) / (double)N;
+            inv_t[i] = 1.0 / (c0 * exp(-2.0 * pi * pi * sigma * sigma * nu * nu));
+        }
+    }
+    cudaError_t e = cudaMalloc((void**)&p->inv_taper_dev, sizeof(double) * (size_t)N);
+    if (e == cudaSuccess) e = cudaMemcpy(p->inv_taper_dev, inv_t, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice);
+    free(inv_t);
+    if (e != cudaSuccess) {
+        if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
+        delete p;
+        return e == cudaErrorMemoryAllocation ? RICK_ENOMEM : RICK_ECUDA;
+    }
+    for (int i = 0; i < RICK_T_COUNT; ++i) {
+        if (cudaEventCreate(&p->ev_start[i]) != cudaSuccess || cudaEventCreate(&p->ev_stop[i]) != cudaSuccess) {
+            rick_plan_destroy(p);
+            return RICK_ECUDA;
+        }
+    }
+    *out = p;
+    return RICK_OK;
+}
+
+int rick_plan_set_dtype(rick_plan* p, int dtype) {
+    if (!p || (dtype != RICK_C64 && dtype != RICK_C128)) return RICK_EINVAL;
+    p->dtype = dtype;
+    p->dtype_set = true;
+    return build_fft(p);
+}
+
+int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes, size_t* fft_bytes) {
+    if (!p || M < 0 || M >= 4294967295ll) return RICK_EINVAL;
+    if (bin_bytes) *bin_bytes = rick_bin_workspace_bytes(p, M);
+    if (fft_bytes) {
+        if (!p->fft_ready) return RICK_ESTATE;
+        *fft_bytes = p->fft_work_bytes;
+    }
+    return RICK_OK;
+}
+
+int rick_plan_destroy(rick_plan* p) {
+    if (!p) return RICK_EINVAL;
+    destroy_fft(p);
+    if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
+    for (int i = 0; i < RICK_T_COUNT; ++i) {
+        if (p->ev_start[i]) cudaEventDestroy(p->ev_start[i]);
+        if (p->ev_stop[i]) cudaEventDestroy(p->ev_stop[i]);
+    }
+    delete p;
+    return RICK_OK;
+}
+
+int rick_bin(rick_plan* p, long long M, const float* u, const float* v, const float* w, const void* vis,
+             const float* weight, float* u_s, float* v_s, float* w_s, void* vis_s, float* weight_s,
+             unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out, void* workspace,
+             size_t workspace_bytes, long long* n_kept_dev, void* stream) {
+    if (!p || M < 0 || M >= 4294967295ll || !n_kept_dev) return RICK_EINVAL;
+    if (M > 0 && (!u || !v || !w || !vis || !weight || !u_s || !v_s || !w_s || !vis_s || !weight_s)) return RICK_EINVAL;
+    if (!workspace || ((uintptr_t)workspace & 255)) return RICK_EINVAL;
+    if (workspace_bytes < rick_bin_workspace_bytes(p, M)) return RICK_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    StageTimer tm(p, RICK_T_BIN, st);
+    return rick_bin_impl(p, M, u, v, w, (const float2*)vis, weight, u_s, v_s, w_s, (float2*)vis_s, weight_s,
+                         key_out, perm_out, bin_start_out, workspace, workspace_bytes, n_kept_dev, st);
+}
+
+int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
+    if (!p || !grid) return RICK_EINVAL;
+    if (!p->bound) return RICK_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (zero_first) {
+        StageTimer tz(p, RICK_T_ZERO, st);
+        const size_t cell = (p->dtype == RICK_C128) ? 16 : 8;
+        RICK_CUDA(cudaMemsetAsync(grid, 0, cell * (size_t)p->g.Nw * (size_t)p->g.N * (size_t)p->g.N, st));
+        p->launches++;
+    }
+    StageTimer tm(p, RICK_T_GRID, st);
+    return rick_grid_impl(p, grid, st);
+}
+
+int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_bytes, void* stream) {
+    if (!p || !grid) return RICK_EINVAL;
+    if (!p->fft_ready) return RICK_ESTATE;
+    if (p->fft_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_work_bytes)) return RICK_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cufftSetStream(p->fft, st) != CUFFT_SUCCESS) return RICK_ECUFFT;
+    if (p->fft_work_bytes > 0 && cufftSetWorkArea(p->fft, fft_work) != CUFFT_SUCCESS) return RICK_ECUFFT;
+    StageTimer tm(p, RICK_T_FFT, st);
+    const size_t plane = (size_t)p->g.N * (size_t)p->g.N;
+    for (int k = 0; k < p->g.Nw; k += p->fft_batch) {
+        cufftResult r;
+        if (p->dtype == RICK_C128) {
+            cufftDoubleComplex* d = (cufftDoubleComplex*)grid + plane * (size_t)k;
+            r = cufftExecZ2Z(p->fft, d, d, CUFFT_INVERSE);
+        } else {
+            cufftComplex* d = (cufftComplex*)grid + plane * (size_t)k;
+            r = cufftExecC2C(p->fft, d, d, CUFFT_INVERSE);
+        }
+        if (r != CUFFT_SUCCESS) return RICK_ECUFFT;
+        p->launches++;
+    }
+    return RICK_OK;
+}
+
+int rick_wcorrect_accumulate(rick_plan* p, const void* grid, double* image, int zero_first, void* stream) {
+    if (!p || !grid || !image) return RICK_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    StageTimer tm(p, RICK_T_WCORRECT, st);
+    return rick_wcorrect_impl(p, grid, image, zero_first, st);
+}
+
+int rick_image(rick_plan* p, const double* image_dev, double* out, int out_is_host, void* stream) {
+    if (!p || !image_dev || !out) return RICK_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    StageTimer tm(p, RICK_T_IMAGE, st);
+    const size_t bytes = sizeof(double) * (size_t)p->g.N * (size_t)p->g.N;
+    if (out == image_dev) return RICK_OK;
+    RICK_CUDA(cudaMemcpyAsync(out, image_dev, bytes, out_is_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+    return RICK_OK;
+}
+
+int rick_image_from_host(rick_plan* p, long long M, const float* u_h, const float* v_h, const float* w_h,
+                         const void* vis_h, const float* weight_h, const rick_device_buffers* d,
+                         double* image_host, void* stream) {
+    if (!p || !d || !image_host || M < 0) return RICK_EINVAL;
+    if (M > 0 && (!u_h || !v_h || !w_h || !vis_h || !weight_h)) return RICK_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t m = (size_t)M;
+    if (M > 0) {
+        RICK_CUDA(cudaMemcpyAsync(d->u, u_h, 4 * m, cudaMemcpyHostToDevice, st));
+        RICK_CUDA(cudaMemcpyAsync(d->v, v_h, 4 * m, cudaMemcpyHostToDevice, st));
+        RICK_CUDA(cudaMemcpyAsync(d->w, w_h, 4 * m, cudaMemcpyHostToDevice, st));
+        RICK_CUDA(cudaMemcpyAsync(d->vis, vis_h, 8 * m, cudaMemcpyHostToDevice, st));
+        RICK_CUDA(cudaMemcpyAsync(d->weight, weight_h, 4 * m, cudaMemcpyHostToDevice, st));
+    }
+    int rc = rick_bin(p, M, d->u, d->v, d->w, d->vis, d->weight, d->u_s, d->v_s, d->w_s, d->vis_s, d->weight_s,
+                      NULL, NULL, NULL, d->workspace, d->workspace_bytes, d->n_kept, stream);
+    if (rc != RICK_OK) return rc;
+    if ((rc = rick_grid(p, d->grid, 1, stream)) != RICK_OK) return rc;
+    if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
+    if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
+    if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;
+    RICK_CUDA(cudaStreamSynchronize(st));
+    return RICK_OK;
+}
+
+int rick_get_timings(rick_plan* p, double* ms, int n) {
+    if (!p || !ms || n < 0 || n > RICK_T_COUNT) return RICK_EINVAL;
+    for (int i = 0; i < n; ++i) {
+        ms[i] = 0.0;
+        if (!p->ev_valid[i]) continue;
+        RICK_CUDA(cudaEventSynchronize(p->ev_stop[i]));
+        float t = 0.f;
+        RICK_CUDA(cudaEventElapsedTime(&t, p->ev_start[i], p->ev_stop[i]));
+        ms[i] = (double)t;
+    }
+    return RICK_OK;
+}
+
+long long rick_launch_count(const rick_plan* p) { return p ? p->launches : 0; }
+
+const char* rick_strerror(int status) {
+    switch (status) {
+        case RICK_OK: return "ok";
+        case RICK_EINVAL: return "invalid argument";
+        case RICK_ENOMEM: return "workspace too small or allocation failed";
+        case RICK_ECUDA: return "CUDA runtime error";
+        case RICK_ECUFFT: return "cuFFT error";
+        case RICK_ESTATE: return "call order violated (bind/dtype missing)";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

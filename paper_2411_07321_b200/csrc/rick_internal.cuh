@@ -1,0 +1,107 @@
+// Internal definitions shared by the translation units of librick_b200 (sm_100a only).
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+
+#include "rick_b200.h"
+
+#define RICK_TILE 32          // uv tile edge of the sort key (BASELINE.json north_star (2))
+#define RICK_MAX_PASSES 4
+#define RICK_RADIX_BITS_MAX 8
+
+// Geometry constants handed to kernels by value.
+struct RickGeom {
+    int N, Nw, S, h, T;
+    double s;        // (double)N * dl                      [D2]
+    double half;     // (double)(N/2)
+    double w_min, w_max;
+    double inv_dw;   // (double)Nw / (w_max - w_min)         [D3]
+    double dl;
+    double dw;       // (w_max - w_min) / Nw
+    double sigma;
+    uint32_t n_bins; // Nw * T * T, also the sentinel key      [D4]
+};
+
+struct rick_plan {
+    RickGeom g;
+    int dtype;
+    bool dtype_set;
+    // sort layout
+    int key_bits, n_pass;
+    int digit_bits[RICK_MAX_PASSES], digit_shift[RICK_MAX_PASSES];
+    // taper: inv_t[p] = 1 / t[p], device double[N]
+    double* inv_taper_dev;
+    // cuFFT
+    cufftHandle fft;
+    bool fft_ready;
+    int fft_batch;           // planes per exec call
+    size_t fft_work_bytes;
+    // binding made by rick_bin
+    bool bound;
+    long long M;
+    const float *u_s, *v_s, *w_s, *weight_s;
+    const void* vis_s;
+    const long long* n_kept_dev;
+    // stage timing
+    cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
+    bool ev_valid[RICK_T_COUNT];
+    long long launches;
+    int sm_count;
+};
+
+#define RICK_CUDA(call)                                  \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return RICK_ECUDA;        \
+    } while (0)
+
+#define RICK_LAUNCH_CHECK()                              \
+    do {                                                 \
+        if (cudaPeekAtLastError() != cudaSuccess) {      \
+            return RICK_ECUDA;                           \
+        }                                                \
+    } while (0)
+
+static inline size_t rick_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---- device helpers --------------------------------------------------------------------------
+
+// D2/D3/D5 with explicitly rounded fp64 operations (never contracted), so that the indices are
+// bit-identical to any other correctly rounded evaluation of the same rules.
+struct RickLoc {
+    double x, y;
+    int i0, j0, k;
+    bool keep;
+};
+
+__device__ __forceinline__ bool rick_finite(float a) { return fabsf(a) <= 3.402823466e+38f; }
+
+__device__ __forceinline__ RickLoc rick_locate(const RickGeom& g, float u, float v, float w) {
+    RickLoc r;
+    r.x = __fma_rn((double)u, g.s, g.half);
+    r.y = __fma_rn((double)v, g.s, g.half);
+    const double xr = floor(__dadd_rn(r.x, 0.5));
+    const double yr = floor(__dadd_rn(r.y, 0.5));
+    const double lo = (double)g.h, hi = (double)(g.N - 1 - g.h);
+    const double t = __dmul_rn(__dsub_rn((double)w, g.w_min), g.inv_dw);
+    double kf = floor(t);
+    if (kf >= (double)g.Nw && (double)w <= g.w_max) kf = (double)(g.Nw - 1);
+    r.keep = (xr >= lo) && (xr <= hi) && (yr >= lo) && (yr <= hi) && (kf >= 0.0) && (kf < (double)g.Nw);
+    r.i0 = r.keep ? (int)xr : 0;
+    r.j0 = r.keep ? (int)yr : 0;
+    r.k = r.keep ? (int)kf : 0;
+    return r;
+}
+
+// translation-unit entry points (host side)
+int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, const float* w,
+                  const float2* vis, const float* weight, float* u_s, float* v_s, float* w_s,
+                  float2* vis_s, float* weight_s, unsigned* key_out, unsigned* perm_out,
+                  unsigned long long* bin_start_out, void* workspace, size_t workspace_bytes,
+                  long long* n_kept_dev, cudaStream_t st);
+size_t rick_bin_workspace_bytes(const rick_plan* p, long long M);
+int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st);
+int rick_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);

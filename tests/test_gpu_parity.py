@@ -1,0 +1,249 @@
+"""GPU parity: the CUDA path, called through the C ABI (ctypes binding), against the CPU oracle on the
+same seeded inputs.  Integer work (keys, plane indices, stable permutation, bin offsets, n_kept) is
+bit-exact; images are gated as DESIGN.md "Parity gate" states (BASELINE.json north_star tolerances:
+1e-5 x peak for the fp32 mesh, 1e-10 x peak for the fp64 mesh)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import rick_oracle as O
+from paper_2411_07321_b200 import binding as B
+from paper_2411_07321_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c64": 1e-5, "c128": 1e-10}
+
+
+def gates(img, ref, N, support, sigma):
+    """-> (gate A, gate B, full-image) max abs differences relative to the inner-half peak."""
+    t = O.taper(N, support, sigma)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    inner = slice(N // 4, 3 * N // 4)
+    peak = np.abs(ref[inner, inner]).max()
+    d = np.abs(img - ref)
+    return d[tw >= 1e-2].max() / peak, (d * tw).max() / peak, d.max() / peak
+
+
+def make(cfg_name, M, device="cuda", **plan):
+    cfg = W.scaled(W.CONFIGS[cfg_name], M, **plan)
+    vis = W.generate(cfg, device=device)
+    pa = W.plan_args(cfg, vis)
+    return cfg, vis, pa
+
+
+def run_bin(im, vis):
+    M = vis.M
+    key = torch.empty(max(M, 1), dtype=torch.int32, device="cuda")
+    perm = torch.empty(max(M, 1), dtype=torch.int32, device="cuda")
+    nb = im.Nw * (im.N // 32) ** 2
+    bs = torch.empty(nb + 2, dtype=torch.int64, device="cuda")
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight, key_out=key, perm_out=perm, bin_start_out=bs)
+    torch.cuda.synchronize()
+    return (key[:M].cpu().numpy().view(np.uint32), perm[:M].cpu().numpy().view(np.uint32),
+            bs.cpu().numpy().view(np.uint64), int(im.n_kept.item()))
+
+
+def check_bin(im, vis, pa):
+    u, v, w, vv, wt = vis.numpy()
+    plan = O.Plan(**pa)
+    key, perm, bs, n_kept = run_bin(im, vis)
+    okey, _, _, _, on = O.keys(plan, u, v, w, vv, wt)
+    assert np.array_equal(key, okey)
+    assert n_kept == on
+    operm = O.sort(okey)
+    assert np.array_equal(perm, operm)
+    _, obs = O.counting_sort(okey, plan.n_bins)
+    assert np.array_equal(bs, obs)
+    s = im.sorted
+    sel = operm[:n_kept].astype(np.int64)
+    assert np.array_equal(s["u"][:n_kept].cpu().numpy(), u[sel])
+    assert np.array_equal(s["v"][:n_kept].cpu().numpy(), v[sel])
+    assert np.array_equal(s["w"][:n_kept].cpu().numpy(), w[sel])
+    assert np.array_equal(s["vis"][:n_kept].cpu().numpy(), vv[sel])
+    assert np.array_equal(s["weight"][:n_kept].cpu().numpy(), wt[sel])
+    return okey, operm, n_kept
+
+
+@pytest.mark.parametrize("name,M,plan,dtype", [
+    ("tiny", 100_000, {}, "c128"),
+    ("10M", 300_017, dict(N=512, Nw=8), "c64"),                     # ragged tail, several sort tiles
+    ("10M", 1_000_003, dict(N=2048, Nw=32), "c64"),                 # 18-bit keys, 3 passes
+    ("hotspot", 400_001, dict(N=1024, Nw=4), "c64"),  # support 9, 70 % in a dense core
+])
+def test_bin_bit_exact(name, M, plan, dtype):
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    im = B.Imager(dtype=dtype, M_max=M, **pa)
+    check_bin(im, vis, pa)
+    im.close()
+
+
+def test_sort_many_tiles_and_hot_bin():
+    """Hand-made keys: 40 sort tiles + ragged tail, one bin holding half of the data, sentinels."""
+    N, Nw = 1024, 16
+    pa = dict(N=N, Nw=Nw, support=7, sigma=1.0, w_min=-8.0, w_max=8.0, dl=0.25 / N)
+    M = 40 * 8192 + 4321
+    rng = np.random.default_rng(77)
+    s = N * pa["dl"]
+    u = (rng.uniform(-500, 500, M) / s).astype(np.float32)
+    v = (rng.uniform(-500, 500, M) / s).astype(np.float32)
+    w = rng.uniform(-8.5, 8.5, M).astype(np.float32)          # some out of range
+    hot = rng.random(M) < 0.5
+    u[hot] = (rng.uniform(3, 20, hot.sum()) / s).astype(np.float32)
+    v[hot] = (rng.uniform(3, 20, hot.sum()) / s).astype(np.float32)
+    w[hot] = 0.3
+    u[::1001] = 1e9                                              # off the mesh
+    t = lambda a: torch.from_numpy(a).cuda()
+    vis = W.Visibilities(t(u), t(v), t(w), torch.ones(M, dtype=torch.complex64, device="cuda"),
+                         torch.ones(M, dtype=torch.float32, device="cuda"))
+    im = B.Imager(dtype="c64", M_max=M, **pa)
+    okey, _, n_kept = check_bin(im, vis, pa)
+    assert 0 < n_kept < M and len(np.unique(okey)) > 2000
+    im.close()
+
+
+@pytest.mark.parametrize("name,M,plan,dtype", [
+    ("tiny", 100_000, {}, "c128"),                                   # BASELINE.json configs[0], full size
+    ("tiny", 100_000, {}, "c64"),
+    ("10M", 500_000, dict(N=512, Nw=8), "c64"),
+    ("100M", 400_000, dict(N=512, Nw=16), "c128"),                  # wide field: the w term matters
+    ("hotspot", 400_001, dict(N=1024, Nw=4), "c64"),  # support 9, sigma 1.3
+])
+def test_stages_and_image(name, M, plan, dtype):
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    N, Nw = pa["N"], pa["Nw"]
+    oplan = O.Plan(**pa)
+    hv = vis.numpy()
+    im = B.Imager(dtype=dtype, M_max=M, **pa)
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
+    # --- gridding: the modulated mesh times the checkerboard is Eq. 3
+    im.grid_(True)
+    torch.cuda.synchronize()
+    ii = np.arange(N)
+    cb = np.where((ii[:, None] + ii[None, :]) & 1, -1.0, 1.0)
+    g = im.grid.cpu().numpy().astype(np.complex128) * cb[None]
+    og = O.grid(oplan, *hv)
+    scale = np.abs(og).max()
+    gerr = np.abs(g - og).max() / scale
+    assert gerr <= (1e-13 if dtype == "c128" else 2e-6), gerr
+    # centre-pixel invariant on the GPU mesh (needs no FFT)
+    t = O.taper(N, cfg.support, cfg.sigma)
+    # --- plane transform (cuFFT) against the oracle's own FFT, plane by plane
+    im.fft()
+    torch.cuda.synchronize()
+    P = im.grid.cpu().numpy().astype(np.complex128) * cb[None]
+    for k in {0, Nw // 2, Nw - 1}:
+        oP = O.plane_transform(og[k])
+        ref_scale = max(np.abs(oP).max(), 1e-300)
+        perr = np.abs(P[k] - oP).max() / max(ref_scale, scale)
+        assert perr <= (1e-12 if dtype == "c128" else 5e-6) * max(1.0, np.log2(N)), perr
+    # --- image
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    img = im.image.cpu().numpy()
+    ref = O.image(oplan, *hv)
+    a, b, full = gates(img, ref, N, cfg.support, cfg.sigma)
+    print(f"{name}/{dtype} N={N} Nw={Nw}: grid {gerr:.2e} gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
+    assert a <= TOL[dtype], a
+    assert b <= TOL[dtype], b
+    centre = img[N // 2, N // 2] * t[N // 2] ** 2
+    assert abs(centre - og.sum().real) <= (1e-11 if dtype == "c128" else 1e-5) * np.abs(og).sum()
+    im.close()
+
+
+def test_full_config_10M_image():
+    """BASELINE.json configs[1] at full size, in the configuration bench.py times."""
+    cfg, vis, pa = make("10M", W.CONFIGS["10M"].M)
+    im = B.Imager(dtype="c64", M_max=vis.M, **pa)
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy()
+    ref, n_kept, _ = O.image(O.Plan(**pa), *vis.numpy(), return_timing=True)
+    assert int(im.n_kept.item()) == n_kept
+    a, b, full = gates(img, ref, cfg.N, cfg.support, cfg.sigma)
+    print(f"10M full: n_kept={n_kept} gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
+    assert a <= TOL["c64"] and b <= TOL["c64"]
+    im.close()
+
+
+def test_edge_cases():
+    pa = dict(N=256, Nw=8, support=7, sigma=1.0, w_min=-100.0, w_max=100.0, dl=0.2 / 256)
+    oplan = O.Plan(**pa)
+    im = B.Imager(dtype="c128", M_max=16, **pa)
+    z32 = lambda n: torch.zeros(n, dtype=torch.float32, device="cuda")
+    # empty input
+    e = W.Visibilities(z32(0), z32(0), z32(0), torch.zeros(0, dtype=torch.complex64, device="cuda"), z32(0))
+    img = im.run(e.u, e.v, e.w, e.vis, e.weight)
+    torch.cuda.synchronize()
+    assert int(im.n_kept.item()) == 0 and float(img.abs().max()) == 0.0
+    # all dropped: off-mesh, out of w range, NaN / Inf in every field
+    u = torch.tensor([1e9, 0, 0, float("nan"), 0, 0, 0], dtype=torch.float32, device="cuda")
+    v = torch.tensor([0, -1e9, 0, 0, float("inf"), 0, 0], dtype=torch.float32, device="cuda")
+    w = torch.tensor([0, 0, 101.0, 0, 0, 0, 0], dtype=torch.float32, device="cuda")
+    vv = torch.ones(7, dtype=torch.complex64, device="cuda")
+    vv[5] = complex(float("nan"), 0.0)
+    wt = torch.ones(7, dtype=torch.float32, device="cuda")
+    wt[6] = float("inf")
+    img = im.run(u, v, w, vv, wt)
+    torch.cuda.synchronize()
+    assert int(im.n_kept.item()) == 0 and float(img.abs().max()) == 0.0
+    # the hand cases of tests/golden (edges, ties, w == w_max): keys and image
+    import os
+    rows = [l.split("#")[0].split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "keys_hand_cases.txt"))]
+    rows = [r for r in rows if r]
+    u = torch.tensor([float(r[0]) for r in rows], dtype=torch.float32, device="cuda")
+    v = torch.tensor([float(r[1]) for r in rows], dtype=torch.float32, device="cuda")
+    w = torch.tensor([float(r[2]) for r in rows], dtype=torch.float32, device="cuda")
+    n = len(rows)
+    vis = W.Visibilities(u, v, w, torch.full((n,), 1 + 0.5j, dtype=torch.complex64, device="cuda"),
+                         torch.ones(n, dtype=torch.float32, device="cuda"))
+    key, perm, bs, n_kept = run_bin(im, vis)
+    T = pa["N"] // 32
+    exp = [oplan.n_bins if int(r[5]) < 0 else (int(r[5]) * T + (int(r[4]) >> 5)) * T + (int(r[3]) >> 5) for r in rows]
+    assert list(key) == exp
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy()
+    ref = O.image(oplan, *vis.numpy())
+    a, b, _ = gates(img, ref, 256, 7, 1.0)
+    assert a <= 1e-10 and b <= 1e-10
+    im.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_input_order_invariance(dtype):
+    cfg, vis, pa = make("10M", 200_000, N=512, Nw=8, dtype=dtype)
+    im = B.Imager(dtype=dtype, M_max=vis.M, **pa)
+    a = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    g = torch.Generator(device="cpu").manual_seed(5)
+    p = torch.randperm(vis.M, generator=g).cuda()
+    b = im.run(vis.u[p].contiguous(), vis.v[p].contiguous(), vis.w[p].contiguous(), vis.vis[p].contiguous(),
+               vis.weight[p].contiguous()).cpu().numpy()
+    t = O.taper(cfg.N, cfg.support, cfg.sigma)
+    tw = np.outer(t, t) / t[cfg.N // 2] ** 2
+    peak = np.abs(a * tw).max()
+    assert (np.abs(a - b) * tw).max() <= (1e-12 if dtype == "c128" else 1e-5) * peak
+    im.close()
+
+
+def test_chunked_accumulation_and_host_entry():
+    """rick_grid(zero_first=0) accumulates chunks; rick_image_from_host equals the device path."""
+    cfg, vis, pa = make("10M", 120_000, N=512, Nw=8, dtype="c128")
+    im = B.Imager(dtype="c128", M_max=vis.M, **pa)
+    whole = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    half = vis.M // 2
+    parts = [slice(0, half), slice(half, vis.M)]
+    for n, sl in enumerate(parts):
+        im.bin(vis.u[sl].contiguous(), vis.v[sl].contiguous(), vis.w[sl].contiguous(), vis.vis[sl].contiguous(),
+               vis.weight[sl].contiguous())
+        im.grid_(zero_first=(n == 0))
+    im.fft()
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    chunked = im.image.cpu().numpy()
+    t = O.taper(cfg.N, cfg.support, cfg.sigma)
+    tw = np.outer(t, t) / t[cfg.N // 2] ** 2
+    assert (np.abs(chunked - whole) * tw).max() <= 1e-12 * np.abs(whole * tw).max()
+    host = [x.cpu().pin_memory() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
+    out = torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory()
+    im.run_from_host(*host, out)
+    assert (np.abs(out.numpy() - whole) * tw).max() <= 1e-12 * np.abs(whole * tw).max()
+    tm = im.timings()
+    assert all(tm[k] > 0 for k in ("bin", "zero", "grid", "fft", "wcorrect", "image"))
+    im.close()
