@@ -58,7 +58,9 @@ typedef enum { RICK_C64 = 0, RICK_C128 = 1 } rick_dtype;
 
 /* stage indices of rick_get_timings */
 enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_WCORRECT = 4,
-       RICK_T_IMAGE = 5, RICK_T_COUNT = 6 };
+       RICK_T_IMAGE = 5,
+       /* parts of RICK_T_BIN */
+       RICK_T_KEYGEN = 6, RICK_T_SORT = 7, RICK_T_GATHER = 8, RICK_T_COUNT = 9 };
 
 /* Create a plan (BASELINE.json north_star (1)).  Host-synchronous.
  *   N        mesh and image size per axis; a multiple of 32 (tile size), 32 <= N <= 32768
@@ -148,7 +150,8 @@ int rick_image_from_host(rick_plan* plan, long long M, const float* u_host, cons
  * stages never run report 0.  Synchronises on the recorded events.  n <= RICK_T_COUNT. */
 int rick_get_timings(rick_plan* plan, double* ms, int n);
 
-/* Number of kernel launches (library kernels + cuFFT exec calls) issued through this plan so far. */
+/* Number of launches of the library's own kernels issued through this plan so far (memsets, copies and
+ * cuFFT's internal kernels are not counted). */
 long long rick_launch_count(const rick_plan* plan);
 
 const char* rick_strerror(int status);

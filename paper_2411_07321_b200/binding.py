@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 RICK_C64, RICK_C128 = 0, 1
-RICK_T_NAMES = ("bin", "zero", "grid", "fft", "wcorrect", "image")
+RICK_T_NAMES = ("bin", "zero", "grid", "fft", "wcorrect", "image", "keygen", "sort", "gather")
 
 _lib = None
 

@@ -269,21 +269,19 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
     Workspace ws = carve(workspace, M);
     p->bound = false;
     RICK_CUDA(cudaMemsetAsync(n_kept_dev, 0, sizeof(long long), st));
-    p->launches++;
     if (M == 0) {
         if (bin_start_out) {
             RICK_CUDA(cudaMemsetAsync(bin_start_out, 0, sizeof(unsigned long long) * ((size_t)g.n_bins + 2), st));
-            p->launches++;
         }
     } else {
         RICK_CUDA(cudaMemsetAsync((char*)workspace + ws.zero_offset, 0, ws.zero_bytes, st));
-        p->launches++;
         SortLayout lay;
         lay.n_pass = p->n_pass;
         for (int i = 0; i < RICK_MAX_PASSES; ++i) {
             lay.shift[i] = p->digit_shift[i];
             lay.bits[i] = p->digit_bits[i];
         }
+        rick_stage_begin(p, RICK_T_KEYGEN, st);
         {
             const long long want = (M + 256 * 8 - 1) / (256 * 8);
             const long long cap = (long long)p->sm_count * 16;
@@ -295,8 +293,9 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         }
         if (key_out) {
             RICK_CUDA(cudaMemcpyAsync(key_out, ws.key_a, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
-            p->launches++;
         }
+        rick_stage_end(p, RICK_T_KEYGEN, st);
+        rick_stage_begin(p, RICK_T_SORT, st);
         k_scan_hist<<<p->n_pass, kRadix, 0, st>>>(ws.hist);
         RICK_LAUNCH_CHECK();
         p->launches++;
@@ -318,10 +317,10 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             t = kin; kin = kout; kout = t;
             t = iin; iin = iout; iout = t;
         }
+        rick_stage_end(p, RICK_T_SORT, st);
         // sorted (key, index) now live in kin / iin
         if (perm_out) {
             RICK_CUDA(cudaMemcpyAsync(perm_out, iin, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
-            p->launches++;
         }
         if (bin_start_out) {
             const long long want = (M + 1 + 255) / 256;
@@ -330,6 +329,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             RICK_LAUNCH_CHECK();
             p->launches++;
         }
+        rick_stage_begin(p, RICK_T_GATHER, st);
         {
             const long long want = (M + 255) / 256;
             const long long cap = (long long)p->sm_count * 32;
@@ -338,6 +338,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             RICK_LAUNCH_CHECK();
             p->launches++;
         }
+        rick_stage_end(p, RICK_T_GATHER, st);
     }
     p->M = M;
     p->u_s = u_s; p->v_s = v_s; p->w_s = w_s; p->vis_s = vis_s; p->weight_s = weight_s;

@@ -6,6 +6,12 @@
 
 #include "rick_internal.cuh"
 
+void rick_stage_begin(rick_plan* p, int stage, cudaStream_t st) { cudaEventRecord(p->ev_start[stage], st); }
+void rick_stage_end(rick_plan* p, int stage, cudaStream_t st) {
+    cudaEventRecord(p->ev_stop[stage], st);
+    p->ev_valid[stage] = true;
+}
+
 namespace {
 
 int ceil_log2_u64(unsigned long long v) {   // smallest b with 2^b > v  (bits needed to store v)
@@ -200,7 +206,6 @@ int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
         StageTimer tz(p, RICK_T_ZERO, st);
         const size_t cell = (p->dtype == RICK_C128) ? 16 : 8;
         RICK_CUDA(cudaMemsetAsync(grid, 0, cell * (size_t)p->g.Nw * (size_t)p->g.N * (size_t)p->g.N, st));
-        p->launches++;
     }
     StageTimer tm(p, RICK_T_GRID, st);
     return rick_grid_impl(p, grid, st);
@@ -225,7 +230,6 @@ int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_by
             r = cufftExecC2C(p->fft, d, d, CUFFT_INVERSE);
         }
         if (r != CUFFT_SUCCESS) return RICK_ECUFFT;
-        p->launches++;
     }
     return RICK_OK;
 }

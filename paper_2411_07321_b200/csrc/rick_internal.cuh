@@ -97,6 +97,8 @@ __device__ __forceinline__ RickLoc rick_locate(const RickGeom& g, float u, float
 }
 
 // translation-unit entry points (host side)
+void rick_stage_begin(rick_plan* p, int stage, cudaStream_t st);
+void rick_stage_end(rick_plan* p, int stage, cudaStream_t st);
 int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, const float* w,
                   const float2* vis, const float* weight, float* u_s, float* v_s, float* w_s,
                   float2* vis_s, float* weight_s, unsigned* key_out, unsigned* perm_out,
