@@ -251,7 +251,34 @@ long long rick_oracle_keys(int N, int Nw, int S, double w_min, double w_max, dou
     return kept;
 }
 
-// D4: the stable order (key, input index).  perm[r] = input index of the visibility at sorted rank r.
+// D4': the key rick_bin actually sorts by is the tile key of D4 refined by the
+// in-tile cell index c = (j0 & 31) * 32 + (i0 & 31) (10 bits), so that visibilities sharing a nearest
+// cell are adjacent while the order stays grouped by (plane, tile):
+//     cb       = the largest c <= 10 with  Nw T^2 * 2^c <= 2^32
+//     sort_key = key * 2^cb + (c >> (10 - cb))          kept visibilities
+//     sort_key = min(Nw T^2 * 2^cb, 2^32 - 1)            dropped visibilities (sorts last: when the product
+//                is 2^32 the all-ones value is the last cell of the last tile, which D5 never keeps)
+// key / i0 / j0 are the outputs of rick_oracle_keys.  Returns cb.
+int rick_oracle_sort_key(int N, int Nw, long long M, const uint32_t* key, const int32_t* i0,
+                         const int32_t* j0, uint32_t* sort_key) {
+    const uint64_t T = (uint64_t)(N / 32);
+    const uint64_t n_bins = (uint64_t)Nw * T * T;
+    int cb = 10;
+    while (cb > 0 && (n_bins << cb) > (1ull << 32)) --cb;
+    const uint64_t top = n_bins << cb;
+    const uint32_t sentinel = top > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)top;
+    for (long long m = 0; m < M; ++m) {
+        if ((uint64_t)key[m] >= n_bins) {
+            sort_key[m] = sentinel;
+        } else {
+            const uint64_t c = (uint64_t)(((j0[m] & 31) << 5) | (i0[m] & 31));
+            sort_key[m] = (uint32_t)(((uint64_t)key[m] << cb) | (c >> (10 - cb)));
+        }
+    }
+    return cb;
+}
+
+// D4/D4': the stable order (key, input index).  perm[r] = input index of the visibility at sorted rank r.
 void rick_oracle_sort(long long M, const uint32_t* key, uint32_t* perm) {
     std::iota(perm, perm + M, (uint32_t)0);
     std::stable_sort(perm, perm + M, [key](uint32_t a, uint32_t b) { return key[a] < key[b]; });

@@ -42,6 +42,8 @@ def lib():
         L.rick_oracle_keys.argtypes = geo + [C.c_double, C.c_double, C.c_double, C.c_longlong,
                                              f32p, f32p, f32p, f32p, f32p, u32p, i32p, i32p, i32p]
         L.rick_oracle_sort.argtypes = [C.c_longlong, u32p, u32p]
+        L.rick_oracle_sort_key.restype = C.c_int
+        L.rick_oracle_sort_key.argtypes = [C.c_int, C.c_int, C.c_longlong, u32p, i32p, i32p, u32p]
         L.rick_oracle_counting_sort.argtypes = [C.c_longlong, u32p, C.c_uint32, u32p, u64p]
         L.rick_oracle_grid.argtypes = geo + [C.c_double] * 4 + [C.c_longlong, f32p, f32p, f32p, f32p, f32p, f64p]
         L.rick_oracle_plane_transform.argtypes = [C.c_int, f64p]
@@ -114,6 +116,17 @@ def keys(plan: Plan, u, v, w, vis, wt):
                                _p(vis.view(np.float32), C.c_float), _p(wt, C.c_float),
                                _p(key, C.c_uint32), _p(i0, C.c_int32), _p(j0, C.c_int32), _p(k, C.c_int32))
     return key, i0, j0, k, int(n)
+
+
+def sort_key(plan: Plan, key: np.ndarray, i0: np.ndarray, j0: np.ndarray) -> Tuple[np.ndarray, int]:
+    """D4': -> (sort_key u32[M], cb): the tile key refined by the top cb bits of the in-tile cell index."""
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    i0 = np.ascontiguousarray(i0, dtype=np.int32)
+    j0 = np.ascontiguousarray(j0, dtype=np.int32)
+    out = np.empty(key.shape[0], np.uint32)
+    cb = lib().rick_oracle_sort_key(plan.N, plan.Nw, key.shape[0], _p(key, C.c_uint32), _p(i0, C.c_int32),
+                                    _p(j0, C.c_int32), _p(out, C.c_uint32))
+    return out, int(cb)
 
 
 def sort(key: np.ndarray) -> np.ndarray:

@@ -1,6 +1,10 @@
 // bin.cu -- rick_bin: key generation, hand-written stable LSD radix sort (one-sweep style, decoupled
 // look-back), gather of the SoA payload, optional bin offsets.   [D2-D5], BASELINE.json north_star (2).
 //
+// The key that is sorted is the (w-plane, 32x32 tile) key of D4 refined by the in-tile cell index
+// [D4']: the order is still grouped by plane and tile, and visibilities with the same nearest cell
+// are adjacent, which is what lets rick_grid accumulate whole runs in registers.
+//
 // Passes and traffic per visibility (algorithmic):
 //   K1 keygen+histograms   read 24 B, write 4 B key
 //   K2 one-sweep pass x n_pass (n_pass = ceil(key_bits / 8) <= 3 for the five configs)
@@ -56,7 +60,8 @@ Workspace carve(void* base, long long M) {
 __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const float* __restrict__ u,
                                                 const float* __restrict__ v, const float* __restrict__ w,
                                                 const float2* __restrict__ vis, const float* __restrict__ wt,
-                                                uint32_t* __restrict__ key, uint32_t* __restrict__ hist,
+                                                uint32_t* __restrict__ key, uint32_t* __restrict__ tile_key_out,
+                                                uint32_t* __restrict__ hist,
                                                 unsigned long long* __restrict__ n_kept, SortLayout lay) {
     __shared__ uint32_t sh[RICK_MAX_PASSES][kRadix];
     for (int i = threadIdx.x; i < RICK_MAX_PASSES * kRadix; i += blockDim.x) (&sh[0][0])[i] = 0;
@@ -76,9 +81,10 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
             const bool fin = rick_finite(uu) && rick_finite(vv) && rick_finite(ww) && rick_finite(wgt) &&
                              rick_finite(vi.x) && rick_finite(vi.y);
             const bool keep = r.keep && fin;
-            kk = keep ? (uint32_t)((r.k * g.T + (r.j0 >> 5)) * g.T + (r.i0 >> 5)) : g.n_bins;
+            kk = keep ? rick_sort_key(g, r) : g.sort_sentinel;
             kept += keep ? 1u : 0u;
             key[m] = kk;
+            if (tile_key_out) tile_key_out[m] = keep ? rick_tile_key(g, r) : g.n_bins;
         }
 #pragma unroll
         for (int p = 0; p < RICK_MAX_PASSES; ++p) {
@@ -242,13 +248,14 @@ __global__ void __launch_bounds__(256) k_gather(const long long* __restrict__ n_
     }
 }
 
-// bin_start[b] = number of sorted keys < b, b = 0 .. n_bins + 1
-__global__ void __launch_bounds__(256) k_bin_start(long long M, const uint32_t* __restrict__ key_sorted,
-                                                   uint32_t n_bins, unsigned long long* __restrict__ bin_start) {
+// bin_start[b] = number of sorted tile keys < b, b = 0 .. n_bins + 1
+__global__ void __launch_bounds__(256) k_bin_start(RickGeom g, long long M, const uint32_t* __restrict__ key_sorted,
+                                                   unsigned long long* __restrict__ bin_start) {
+    const uint32_t n_bins = g.n_bins;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i <= M; i += stride) {
-        const long long prev = (i == 0) ? -1ll : (long long)key_sorted[i - 1];
-        const long long cur = (i == M) ? (long long)n_bins + 1 : (long long)key_sorted[i];
+        const long long prev = (i == 0) ? -1ll : (long long)rick_tile_of_sort_key(g, key_sorted[i - 1]);
+        const long long cur = (i == M) ? (long long)n_bins + 1 : (long long)rick_tile_of_sort_key(g, key_sorted[i]);
         for (long long b = prev + 1; b <= cur; ++b) bin_start[b] = (unsigned long long)i;
     }
 }
@@ -286,13 +293,10 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             const long long want = (M + 256 * 8 - 1) / (256 * 8);
             const long long cap = (long long)p->sm_count * 16;
             const int blocks = (int)(want < 1 ? 1 : (want > cap ? cap : want));
-            k_keygen<<<blocks, 256, 0, st>>>(g, M, u, v, w, vis, weight, ws.key_a, ws.hist,
+            k_keygen<<<blocks, 256, 0, st>>>(g, M, u, v, w, vis, weight, ws.key_a, key_out, ws.hist,
                                              (unsigned long long*)n_kept_dev, lay);
             RICK_LAUNCH_CHECK();
             p->launches++;
-        }
-        if (key_out) {
-            RICK_CUDA(cudaMemcpyAsync(key_out, ws.key_a, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
         }
         rick_stage_end(p, RICK_T_KEYGEN, st);
         rick_stage_begin(p, RICK_T_SORT, st);
@@ -325,7 +329,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         if (bin_start_out) {
             const long long want = (M + 1 + 255) / 256;
             const long long cap = (long long)p->sm_count * 16;
-            k_bin_start<<<(int)(want > cap ? cap : want), 256, 0, st>>>(M, kin, g.n_bins, bin_start_out);
+            k_bin_start<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, M, kin, bin_start_out);
             RICK_LAUNCH_CHECK();
             p->launches++;
         }

@@ -1,75 +1,199 @@
 // grid.cu -- rick_grid: convolutional gridding, Eq. 3 with the separable truncated Gaussian [D6].
 //
-// v0 (first correct path): one thread per sorted visibility, S*S vector reductions straight into the
-// mesh in L2 (red.global.add).  Sorted order keeps the reductions of a warp inside one 32x32 tile.
+// Run-accumulating gridder.  rick_bin leaves the kept visibilities sorted by (plane, tile, cell) [D4'],
+// so visibilities that share a nearest cell (i0, j0, k) -- and therefore the same S x S footprint --
+// are adjacent: 87 % of the "10M" workload sits in runs of >= 8.
+// Each thread walks kRunItems consecutive sorted visibilities and keeps the whole footprint
+// (S*S complex accumulators, or a block of RB rows of it per pass) in registers:
+//
+//     acc[b][a] += gx[a] * (gy[b] * weight * V)          2 FMAs per cell and visibility
+//
+// and only when the nearest cell changes (or its range ends) adds the footprint to the mesh with
+// vector reductions in L2 (red.global.add.v2.f32 / red.global.add.f64).  Lanes of a warp hold
+// neighbouring cells, so those reductions fall into the same few sectors.  No shared memory, no
+// shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on sm_100a), and the number
+// of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to kRunItems).
+//
+// The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) depends only on the target cell and
+// is applied once at the flush.
 #include "rick_internal.cuh"
 
 namespace {
 
-constexpr int kMaxS = 15;
+constexpr int kRunThreads = 128;
+constexpr int kRunItems = 16;   // consecutive sorted visibilities per thread (a multiple of 4)
 
-__device__ __forceinline__ void red_add_v2(float2* addr, float a, float b) {
-    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b) : "memory");
+struct TapConst {
+    double K[8];   // K[t] = exp(-t^2 / (2 sigma^2)), t = 0 .. h
+};
+
+__device__ __forceinline__ void red_add_cell(float2* addr, float re, float im) {
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(re), "f"(im) : "memory");
+}
+__device__ __forceinline__ void red_add_cell(double2* addr, double re, double im) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(re) : "memory");
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"((double*)addr + 1), "d"(im) : "memory");
 }
 
-// Taps of one axis: g(i0 + a - x) for a = -h..h, with the checkerboard sign (-1)^(i0+a) folded in
-// (modulated mesh, see rick_b200.h).  d0 = i0 - x is formed in fp64 and narrowed once.
-template <typename real>
-__device__ __forceinline__ void taps(real* t, int S, int h, int i0, double x, real inv_2s2) {
-    const real d0 = (real)((double)i0 - x);
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Taps of one axis, t[a] = g(d0 + a - h), a = 0 .. S-1, d0 = i0 - x (formed in fp64, narrowed once).
+// fp32: one MUFU.EX2 per tap.
+template <int S>
+__device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst&) {
+    constexpr int h = (S - 1) / 2;
+    const float c2 = (float)(-g.tap_c * 1.4426950408889634);   // -log2(e) / (2 sigma^2)
+    const float d = (float)d0;
+#pragma unroll
     for (int a = 0; a < S; ++a) {
-        const real d = d0 + (real)(a - h);
-        real val = (sizeof(real) == 4) ? (real)expf(-(float)(d * d) * (float)inv_2s2) : (real)exp(-(double)(d * d) * (double)inv_2s2);
-        t[a] = ((i0 + a - h) & 1) ? -val : val;
+        const float da = d + (float)(a - h);
+        t[a] = ex2_approx(da * da * c2);
+    }
+}
+// fp64: g(d0 + s) = g(d0) E^s K[|s|] with E = exp(-d0 / sigma^2): two exp and one reciprocal per axis.
+template <int S>
+__device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, const TapConst& tc) {
+    constexpr int h = (S - 1) / 2;
+    const double g0 = exp(-d0 * d0 * g.tap_c);
+    const double E = exp(-2.0 * d0 * g.tap_c);
+    const double Ei = 1.0 / E;
+    t[h] = g0;
+    double pp = g0, pm = g0;
+#pragma unroll
+    for (int s = 1; s <= h; ++s) {
+        pp *= E;
+        pm *= Ei;
+        t[h + s] = pp * tc.K[s];
+        t[h - s] = pm * tc.K[s];
     }
 }
 
-template <typename real, typename cell>
-__global__ void __launch_bounds__(128) k_grid_naive(RickGeom g, const long long* __restrict__ n_kept,
-                                                     const float* __restrict__ u_s, const float* __restrict__ v_s,
-                                                     const float* __restrict__ w_s, const float2* __restrict__ vis_s,
-                                                     const float* __restrict__ wt_s, cell* __restrict__ grid) {
+template <typename real> struct CellOf;
+template <> struct CellOf<float> { typedef float2 type; };
+template <> struct CellOf<double> { typedef double2 type; };
+
+// four consecutive floats starting at p (p is a multiple of 4); entries at or beyond n are not read
+__device__ __forceinline__ float4 load4(const float* __restrict__ a, long long p, long long n) {
+    if (p + 4 <= n) return __ldg((const float4*)(a + p));
+    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (p < n) r.x = __ldg(a + p);
+    if (p + 1 < n) r.y = __ldg(a + p + 1);
+    if (p + 2 < n) r.z = __ldg(a + p + 2);
+    return r;
+}
+
+template <typename real, int S, int RB>
+__global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
+                                                          const float* __restrict__ u_s, const float* __restrict__ v_s,
+                                                          const float* __restrict__ w_s, const float2* __restrict__ vis_s,
+                                                          const float* __restrict__ wt_s,
+                                                          typename CellOf<real>::type* __restrict__ grid) {
+    typedef typename CellOf<real>::type cell;
+    constexpr int h = (S - 1) / 2;
+    constexpr int kPasses = (S + RB - 1) / RB;
     const long long n = *n_kept;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    const real inv_2s2 = (real)(1.0 / (2.0 * g.sigma * g.sigma));
-    for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += stride) {
-        const RickLoc r = rick_locate(g, u_s[m], v_s[m], w_s[m]);
-        const float2 vi = vis_s[m];
-        const float wgt = wt_s[m];
-        const real vr = (real)wgt * (real)vi.x, vim = (real)wgt * (real)vi.y;
-        real gx[kMaxS], gy[kMaxS];
-        taps<real>(gx, g.S, g.h, r.i0, r.x, inv_2s2);
-        taps<real>(gy, g.S, g.h, r.j0, r.y, inv_2s2);
-        cell* base = grid + ((size_t)r.k * g.N + (size_t)(r.j0 - g.h)) * g.N + (size_t)(r.i0 - g.h);
-        for (int b = 0; b < g.S; ++b) {
-            const real yr = gy[b] * vr, yi = gy[b] * vim;
-            cell* row = base + (size_t)b * g.N;
-            for (int a = 0; a < g.S; ++a) {
-                if (sizeof(real) == 4) {
-                    red_add_v2((float2*)(row + a), (float)(gx[a] * yr), (float)(gx[a] * yi));
-                } else {
-                    double* c = (double*)(row + a);
-                    atomicAdd(c, (double)(gx[a] * yr));
-                    atomicAdd(c + 1, (double)(gx[a] * yi));
+    const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * kRunItems;
+    if (first >= n) return;
+    const size_t N = (size_t)g.N;
+
+#pragma unroll
+    for (int pass = 0; pass < kPasses; ++pass) {
+        constexpr int dummy = 0;
+        (void)dummy;
+        const int b0 = pass * RB;
+        real ar[RB][S], ai[RB][S];
+#pragma unroll
+        for (int r = 0; r < RB; ++r)
+#pragma unroll
+            for (int a = 0; a < S; ++a) ar[r][a] = ai[r][a] = (real)0;
+        int ci = -1, cj = 0, ck = 0;
+
+        auto flush = [&]() {
+            cell* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)(ci - h);
+            const real s0 = ((ci + cj) & 1) ? (real)-1 : (real)1;
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                if (b0 + r < S) {
+#pragma unroll
+                    for (int a = 0; a < S; ++a) {
+                        const real sg = ((a + b0 + r) & 1) ? -s0 : s0;
+                        red_add_cell(base + (size_t)r * N + a, ar[r][a] * sg, ai[r][a] * sg);
+                        ar[r][a] = ai[r][a] = (real)0;
+                    }
                 }
             }
+        };
+
+        auto one = [&](float uu, float vv, float ww, float re, float im, float wgt) {
+            const RickLoc loc = rick_locate(g, uu, vv, ww);
+            if (loc.i0 != ci || loc.j0 != cj || loc.k != ck) {
+                if (ci >= 0) flush();
+                ci = loc.i0; cj = loc.j0; ck = loc.k;
+            }
+            real gx[S], gy[S];
+            taps<S>(gx, (double)loc.i0 - loc.x, g, tc);
+            taps<S>(gy, (double)loc.j0 - loc.y, g, tc);
+            const real vr = (real)wgt * (real)re, vi = (real)wgt * (real)im;
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                if (b0 + r < S) {
+                    const real yr = gy[b0 + r] * vr, yi = gy[b0 + r] * vi;
+#pragma unroll
+                    for (int a = 0; a < S; ++a) {
+                        ar[r][a] = fma(gx[a], yr, ar[r][a]);
+                        ai[r][a] = fma(gx[a], yi, ai[r][a]);
+                    }
+                }
+            }
+        };
+
+#pragma unroll 1
+        for (int i = 0; i < kRunItems; i += 4) {
+            const long long p = first + i;
+            if (p >= n) break;
+            const float4 u4 = load4(u_s, p, n), v4 = load4(v_s, p, n), w4 = load4(w_s, p, n), t4 = load4(wt_s, p, n);
+            const float4 va = load4((const float*)vis_s, 2 * p, 2 * n);
+            const float4 vb = load4((const float*)vis_s, 2 * p + 4, 2 * n);
+            one(u4.x, v4.x, w4.x, va.x, va.y, t4.x);
+            if (p + 1 < n) one(u4.y, v4.y, w4.y, va.z, va.w, t4.y);
+            if (p + 2 < n) one(u4.z, v4.z, w4.z, vb.x, vb.y, t4.z);
+            if (p + 3 < n) one(u4.w, v4.w, w4.w, vb.z, vb.w, t4.w);
         }
+        if (ci >= 0) flush();
     }
+}
+
+template <typename real, int S, int RB>
+void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
+    typedef typename CellOf<real>::type cell;
+    TapConst tc;
+    for (int t = 0; t < 8; ++t) tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
+    const long long per_block = (long long)kRunThreads * kRunItems;
+    const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
+    k_grid_runs<real, S, RB><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
+                                                              (const float2*)p->vis_s, p->weight_s, (cell*)grid);
 }
 
 }  // namespace
 
 int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st) {
     if (p->M == 0) return RICK_OK;
-    const long long want = (p->M + 127) / 128;
-    const long long cap = (long long)p->sm_count * 64;
-    const int blocks = (int)(want > cap ? cap : want);
-    if (p->dtype == RICK_C128)
-        k_grid_naive<double, double2><<<blocks, 128, 0, st>>>(p->g, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
-                                                               (const float2*)p->vis_s, p->weight_s, (double2*)grid);
-    else
-        k_grid_naive<float, float2><<<blocks, 128, 0, st>>>(p->g, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
-                                                             (const float2*)p->vis_s, p->weight_s, (float2*)grid);
+    const bool f64 = (p->dtype == RICK_C128);
+    // <real, S, RB>: RB rows of the footprint are held in registers per pass (2*RB*S accumulators)
+    switch (p->g.S) {
+        case 3:  f64 ? launch_runs<double, 3, 3>(p, grid, st)  : launch_runs<float, 3, 3>(p, grid, st); break;
+        case 5:  f64 ? launch_runs<double, 5, 5>(p, grid, st)  : launch_runs<float, 5, 5>(p, grid, st); break;
+        case 7:  f64 ? launch_runs<double, 7, 4>(p, grid, st)  : launch_runs<float, 7, 7>(p, grid, st); break;
+        case 9:  f64 ? launch_runs<double, 9, 3>(p, grid, st)  : launch_runs<float, 9, 5>(p, grid, st); break;
+        case 11: f64 ? launch_runs<double, 11, 2>(p, grid, st) : launch_runs<float, 11, 4>(p, grid, st); break;
+        case 13: f64 ? launch_runs<double, 13, 2>(p, grid, st) : launch_runs<float, 13, 3>(p, grid, st); break;
+        case 15: f64 ? launch_runs<double, 15, 2>(p, grid, st) : launch_runs<float, 15, 3>(p, grid, st); break;
+        default: return RICK_EINVAL;
+    }
     RICK_LAUNCH_CHECK();
     p->launches++;
     return RICK_OK;

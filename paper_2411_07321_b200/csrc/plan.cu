@@ -103,10 +103,19 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     g.dw = (w_max - w_min) / (double)Nw;
     g.sigma = sigma;
     g.n_bins = (uint32_t)n_bins;
+    g.tap_c = 1.0 / (2.0 * sigma * sigma);
+    // D4': as many in-tile cell bits as fit a 32-bit sort key (10 = the exact cell)
+    g.cell_bits = 10;
+    while (g.cell_bits > 0 && ((unsigned long long)n_bins << g.cell_bits) > (1ull << 32)) --g.cell_bits;
+    {
+        const unsigned long long s = (unsigned long long)n_bins << g.cell_bits;
+        // n_bins << cb == 2^32: the all-ones key is the last cell of the last tile, which D5 never keeps
+        g.sort_sentinel = s > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)s;
+    }
     p->dtype = RICK_C64;
 
-    // radix-sort digit layout: keys take values 0 .. n_bins (the sentinel), LSD passes of <= 8 bits
-    p->key_bits = ceil_log2_u64((unsigned long long)n_bins);
+    // radix-sort digit layout: sort keys take values 0 .. sort_sentinel, LSD passes of <= 8 bits
+    p->key_bits = ceil_log2_u64((unsigned long long)g.sort_sentinel);
     if (p->key_bits < 1) p->key_bits = 1;
     p->n_pass = (p->key_bits + RICK_RADIX_BITS_MAX - 1) / RICK_RADIX_BITS_MAX;
     {

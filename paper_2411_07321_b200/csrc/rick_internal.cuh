@@ -22,7 +22,10 @@ struct RickGeom {
     double dl;
     double dw;       // (w_max - w_min) / Nw
     double sigma;
-    uint32_t n_bins; // Nw * T * T, also the sentinel key      [D4]
+    uint32_t n_bins; // Nw * T * T, also the sentinel tile key [D4]
+    int cell_bits;   // cb: in-tile cell bits appended to the tile key in the sort key [D4']
+    uint32_t sort_sentinel;  // sort key of a dropped visibility: min(n_bins << cb, 2^32 - 1)
+    double tap_c;    // 1 / (2 sigma^2)
 };
 
 struct rick_plan {
@@ -94,6 +97,19 @@ __device__ __forceinline__ RickLoc rick_locate(const RickGeom& g, float u, float
     r.j0 = r.keep ? (int)yr : 0;
     r.k = r.keep ? (int)kf : 0;
     return r;
+}
+
+// D4: tile key.  D4': sort key = tile key refined by the top cell_bits of the in-tile cell index
+// (j0 & 31) << 5 | (i0 & 31), so that equal nearest cells become runs in the sorted order.
+__device__ __forceinline__ uint32_t rick_tile_key(const RickGeom& g, const RickLoc& r) {
+    return (uint32_t)((r.k * g.T + (r.j0 >> 5)) * g.T + (r.i0 >> 5));
+}
+__device__ __forceinline__ uint32_t rick_sort_key(const RickGeom& g, const RickLoc& r) {
+    const uint32_t cell = (uint32_t)(((r.j0 & 31) << 5) | (r.i0 & 31));
+    return (rick_tile_key(g, r) << g.cell_bits) | (cell >> (10 - g.cell_bits));
+}
+__device__ __forceinline__ uint32_t rick_tile_of_sort_key(const RickGeom& g, uint32_t sk) {
+    return sk == g.sort_sentinel ? g.n_bins : (sk >> g.cell_bits);
 }
 
 // translation-unit entry points (host side)
