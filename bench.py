@@ -221,11 +221,13 @@ def main():
     l0 = im.launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStart()      # `ncu --profile-from-start off` sees the timed region only
     e0.record()
     for _ in range(args.steps):
         step()
     e1.record()
     torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStop()
     launches = im.launches() - l0
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
@@ -246,10 +248,11 @@ def main():
             per[k].append(tm[k])
     stage_ms = {k: statistics.median(v) for k, v in per.items()}
     peak, peak_src = _peaks()
-    alg = {   # algorithmic bytes per launch (DESIGN.md "Roofline per kernel")
-        "keygen": 28 * M,
-        "sort": (12 + 16 * (im_passes(pa) - 1)) * M,
-        "gather": 4 * n_kept + 48 * n_kept,
+    _, n_pass, _ = B.rick_plan_sort_layout(im.plan)
+    alg = {   # algorithmic bytes per launch (DESIGN.md section 5)
+        "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
+        "sort": (12 + 16 * (n_pass - 1)) * M,        # first pass 4 r + 8 w, later passes 8 r + 8 w
+        "gather": (4 + 32 + 24) * n_kept,            # index + record in, sorted SoA out
         "zero": mesh_bytes,
         "grid": 24 * n_kept,
         "fft": 4 * mesh_bytes,
@@ -301,7 +304,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
-        "config": {"workload": args.config, "M": M, "M_kept": n_kept, "N": cfg.N, "Nw": cfg.Nw,
+        "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
                    "support": cfg.support, "sigma": cfg.sigma, "mesh": cfg.dtype,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs (240 MB) and mesh (1.07 GB) exceed the 126 MB L2; no explicit flush"
@@ -315,12 +318,6 @@ def main():
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
-
-
-def im_passes(pa) -> int:
-    """Radix passes of rick_bin for this plan: ceil(bits(Nw (N/32)^2) / 8)."""
-    n_bins = pa["Nw"] * (pa["N"] // 32) ** 2
-    return (n_bins.bit_length() + 7) // 8
 
 
 if __name__ == "__main__":

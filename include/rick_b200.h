@@ -64,7 +64,7 @@ enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_
 
 /* Create a plan (BASELINE.json north_star (1)).  Host-synchronous.
  *   N        mesh and image size per axis; a multiple of 32 (tile size), 32 <= N <= 32768
- *   Nw       number of w-planes, 1 <= Nw <= 4096, Nw (N/32)^2 < 2^31
+ *   Nw       number of w-planes, 1 <= Nw <= 4096, Nw (N/32)^2 <= 2^27
  *   support  full footprint width S in cells, odd, 3 <= S <= 15  (h = (S-1)/2)
  *   sigma    Gaussian width in cells, > 0
  *   w_min, w_max   w range covered by the Nw planes, w_max > w_min; plane k is centred at
@@ -82,6 +82,10 @@ int rick_plan_set_dtype(rick_plan* plan, int dtype);
 int rick_plan_workspace_bytes(const rick_plan* plan, long long M, size_t* bin_bytes, size_t* fft_bytes);
 
 int rick_plan_destroy(rick_plan* plan);
+
+/* Layout of the key rick_bin sorts by [D4']: total key bits, number of radix passes (digits of <= 9
+ * bits) and the number of in-tile cell bits appended to the tile key.  Any pointer may be NULL. */
+int rick_plan_sort_layout(const rick_plan* plan, int* key_bits, int* n_pass, int* cell_bits);
 
 /* Key generation + stable radix sort + gather.  [D2-D5], BASELINE.json north_star (2).
  *   M                     number of visibilities, 0 <= M < 2^32 - 1

@@ -256,8 +256,9 @@ long long rick_oracle_keys(int N, int Nw, int S, double w_min, double w_max, dou
 // cell are adjacent while the order stays grouped by (plane, tile):
 //     cb       = the largest c <= 10 with  Nw T^2 * 2^c <= 2^32
 //     sort_key = key * 2^cb + (c >> (10 - cb))          kept visibilities
-//     sort_key = min(Nw T^2 * 2^cb, 2^32 - 1)            dropped visibilities (sorts last: when the product
-//                is 2^32 the all-ones value is the last cell of the last tile, which D5 never keeps)
+//     sort_key = Nw T^2 * 2^cb - 1                        dropped visibilities: the largest key, which belongs to
+//                row j0 = N - 1 of the last tile (cb >= 5 keeps all of j0 & 31; Nw T^2 <= 2^27 is required)
+//                and is never kept by D5 since h >= 1; so dropped visibilities sort last, after every kept one
 // key / i0 / j0 are the outputs of rick_oracle_keys.  Returns cb.
 int rick_oracle_sort_key(int N, int Nw, long long M, const uint32_t* key, const int32_t* i0,
                          const int32_t* j0, uint32_t* sort_key) {
@@ -265,8 +266,7 @@ int rick_oracle_sort_key(int N, int Nw, long long M, const uint32_t* key, const 
     const uint64_t n_bins = (uint64_t)Nw * T * T;
     int cb = 10;
     while (cb > 0 && (n_bins << cb) > (1ull << 32)) --cb;
-    const uint64_t top = n_bins << cb;
-    const uint32_t sentinel = top > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)top;
+    const uint32_t sentinel = (uint32_t)((n_bins << cb) - 1);
     for (long long m = 0; m < M; ++m) {
         if ((uint64_t)key[m] >= n_bins) {
             sort_key[m] = sentinel;

@@ -21,6 +21,7 @@ _lib = None
 
 EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
+    "rick_plan_sort_layout",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
@@ -60,6 +61,7 @@ def lib():
         L.rick_plan_set_dtype.argtypes = [vp, i]
         L.rick_plan_workspace_bytes.argtypes = [vp, ll, C.POINTER(sz), C.POINTER(sz)]
         L.rick_plan_destroy.argtypes = [vp]
+        L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
         L.rick_fft_planes.argtypes = [vp, vp, vp, sz, vp]
@@ -115,6 +117,13 @@ def rick_plan_workspace_bytes(plan: int, M: int):
     a, b = C.c_size_t(), C.c_size_t()
     _check(lib().rick_plan_workspace_bytes(plan, M, C.byref(a), C.byref(b)), "rick_plan_workspace_bytes")
     return int(a.value), int(b.value)
+
+
+def rick_plan_sort_layout(plan: int):
+    """-> (key_bits, n_pass, cell_bits) of the sort key [D4']."""
+    a, b, c = C.c_int(), C.c_int(), C.c_int()
+    _check(lib().rick_plan_sort_layout(plan, C.byref(a), C.byref(b), C.byref(c)), "rick_plan_sort_layout")
+    return int(a.value), int(b.value), int(c.value)
 
 
 def rick_plan_destroy(plan: int) -> None:

@@ -6,19 +6,20 @@
 // are adjacent, which is what lets rick_grid accumulate whole runs in registers.
 //
 // Passes and traffic per visibility (algorithmic):
-//   K1 keygen+histograms   read 24 B, write 4 B key
-//   K2 one-sweep pass x n_pass (n_pass = ceil(key_bits / 8) <= 3 for the five configs)
+//   K1 keygen+histograms   read 24 B, write 4 B key + 32 B staging record (one sector per visibility)
+//   K2 one-sweep pass x n_pass (n_pass = ceil(key_bits / 9): 3 for 27-bit keys, 4 for 28-32 bits)
 //                          read 8 B (4 B in the first pass: the index is implicit), write 8 B
-//   K3 gather              read 4 B index + 24 B payload (sector-amplified: random rows), write 24 B
+//   K3 gather              read 4 B index + one 32-B record (random rows), write 24 B
 #include "rick_internal.cuh"
 
 namespace {
 
-constexpr int kRadix = 1 << RICK_RADIX_BITS_MAX;   // 256 digit values at most
-constexpr int kSortThreads = 512;
+constexpr int kRadix = 1 << RICK_RADIX_BITS_MAX;   // 512 digit values at most
+constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;   // 8192 keys per tile
+constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kDigitsPerThread = kRadix / kSortThreads;   // 2
 
 struct SortLayout {
     int n_pass;
@@ -28,6 +29,7 @@ struct SortLayout {
 
 struct Workspace {
     uint32_t *key_a, *key_b, *idx_a, *idx_b;
+    float4* rec;                     // [M][2]: (u, v, w, re), (im, weight, -, -): one 32-B sector per visibility
     uint32_t* hist;                  // [RICK_MAX_PASSES][kRadix] digit counts -> exclusive bases
     uint32_t* ticket;                // [RICK_MAX_PASSES] dynamic tile ids
     unsigned long long* status;      // [n_tiles][kRadix] look-back words
@@ -45,6 +47,7 @@ Workspace carve(void* base, long long M) {
     ws.key_b = (uint32_t*)(b + off); off += rick_align256(4 * m);
     ws.idx_a = (uint32_t*)(b + off); off += rick_align256(4 * m);
     ws.idx_b = (uint32_t*)(b + off); off += rick_align256(4 * m);
+    ws.rec = (float4*)(b + off); off += rick_align256(32 * m);
     ws.zero_offset = off;
     ws.hist = (uint32_t*)(b + off); off += rick_align256(sizeof(uint32_t) * RICK_MAX_PASSES * kRadix);
     ws.ticket = (uint32_t*)(b + off); off += rick_align256(sizeof(uint32_t) * RICK_MAX_PASSES);
@@ -55,13 +58,13 @@ Workspace carve(void* base, long long M) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// K1: keys + global digit histograms of every pass + n_kept
+// K1: sort keys + AoS staging records + global digit histograms of every pass + n_kept
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const float* __restrict__ u,
                                                 const float* __restrict__ v, const float* __restrict__ w,
                                                 const float2* __restrict__ vis, const float* __restrict__ wt,
-                                                uint32_t* __restrict__ key, uint32_t* __restrict__ tile_key_out,
-                                                uint32_t* __restrict__ hist,
+                                                uint32_t* __restrict__ key, float4* __restrict__ rec,
+                                                uint32_t* __restrict__ tile_key_out, uint32_t* __restrict__ hist,
                                                 unsigned long long* __restrict__ n_kept, SortLayout lay) {
     __shared__ uint32_t sh[RICK_MAX_PASSES][kRadix];
     for (int i = threadIdx.x; i < RICK_MAX_PASSES * kRadix; i += blockDim.x) (&sh[0][0])[i] = 0;
@@ -69,14 +72,14 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
     const int lane = threadIdx.x & 31;
     unsigned kept = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    // warp-uniform trip count so that every lane reaches the match instructions
+    // warp-uniform trip count so that every lane reaches the votes
     for (long long base = (long long)blockIdx.x * blockDim.x; base < M; base += stride) {
         const long long m = base + threadIdx.x;
         const bool valid = m < M;
-        uint32_t kk = 0xFFFFFFFFu;
+        uint32_t kk = 0;
         if (valid) {
-            const float uu = u[m], vv = v[m], ww = w[m], wgt = wt[m];
-            const float2 vi = vis[m];
+            const float uu = __ldg(u + m), vv = __ldg(v + m), ww = __ldg(w + m), wgt = __ldg(wt + m);
+            const float2 vi = __ldg(vis + m);
             RickLoc r = rick_locate(g, uu, vv, ww);
             const bool fin = rick_finite(uu) && rick_finite(vv) && rick_finite(ww) && rick_finite(wgt) &&
                              rick_finite(vi.x) && rick_finite(vi.y);
@@ -84,14 +87,22 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
             kk = keep ? rick_sort_key(g, r) : g.sort_sentinel;
             kept += keep ? 1u : 0u;
             key[m] = kk;
+            rec[2 * m] = make_float4(uu, vv, ww, vi.x);
+            rec[2 * m + 1] = make_float4(vi.y, wgt, 0.f, 0.f);
             if (tile_key_out) tile_key_out[m] = keep ? rick_tile_key(g, r) : g.n_bins;
         }
+        // digit histograms: lanes that share lane 0's digit (the common case in the skewed high
+        // digits) are counted with one vote, the rest with one shared-memory atomic each
+        const unsigned act = __ballot_sync(0xffffffffu, valid);
+        const int first = __ffs(act) - 1;
 #pragma unroll
         for (int p = 0; p < RICK_MAX_PASSES; ++p) {
             if (p < lay.n_pass) {
-                const uint32_t d = valid ? ((kk >> lay.shift[p]) & ((1u << lay.bits[p]) - 1u)) : (0x10000u | lane);
-                const unsigned peers = __match_any_sync(0xffffffffu, d);
-                if (valid && lane == (__ffs(peers) - 1)) atomicAdd(&sh[p][d], (uint32_t)__popc(peers));
+                const uint32_t d = (kk >> lay.shift[p]) & ((1u << lay.bits[p]) - 1u);
+                const uint32_t d0 = __shfl_sync(0xffffffffu, d, first);
+                const unsigned same = __ballot_sync(0xffffffffu, valid && d == d0);
+                if (lane == first) atomicAdd(&sh[p][d0], (uint32_t)__popc(same));
+                else if (valid && d != d0) atomicAdd(&sh[p][d], 1u);
             }
         }
     }
@@ -104,7 +115,7 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
     if (lane == 0 && kept) atomicAdd(n_kept, (unsigned long long)kept);
 }
 
-// exclusive scan of each pass's 256 digit counts, in place (one block per pass)
+// exclusive scan of each pass's kRadix digit counts, in place (one block per pass)
 __global__ void __launch_bounds__(kRadix) k_scan_hist(uint32_t* __restrict__ hist) {
     __shared__ uint32_t s[kRadix];
     uint32_t* h = hist + blockIdx.x * kRadix;
@@ -122,9 +133,10 @@ __global__ void __launch_bounds__(kRadix) k_scan_hist(uint32_t* __restrict__ his
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2: one stable LSD pass.  Tiles take their id from a ticket (so that every predecessor is already
-// running), rank their keys per warp with match.any (stable: items are warp-striped and visited in
-// order), publish per-digit tile counts and resolve their global offsets by decoupled look-back.
+// K2: one stable LSD pass (one-sweep).  Tiles take their id from a ticket (so that every predecessor
+// is already running), rank their keys per warp with ballots (stable: items are warp-striped and
+// visited in order), publish per-digit tile counts and resolve their global offsets by decoupled
+// look-back, exchange the tile through shared memory into digit order and write it out in runs.
 // status word: [63:62] state (1 = tile aggregate, 2 = inclusive prefix) | [61:32] epoch | [31:0] count
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long pack_status(uint32_t state, uint32_t epoch, uint32_t value) {
@@ -141,110 +153,194 @@ __device__ __forceinline__ void st_status(unsigned long long* p, unsigned long l
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+struct SortSmem {
+    uint32_t warp_cnt[kSortWarps][kRadix];   // per-warp digit counts -> exclusive offsets over warps
+    uint32_t tile_excl[kRadix];              // first slot of each digit in the exchanged tile
+    uint32_t glob[kRadix];                   // global position of slot i of digit d = glob[d] + i
+    uint32_t xkey[kSortTile];
+    uint32_t xidx[kSortTile];
+    uint32_t warp_sum[kSortWarps];
+    uint32_t tile;
+};
+
 template <bool kFirst>
-__global__ void __launch_bounds__(kSortThreads) k_onesweep(const uint32_t* __restrict__ key_in,
-                                                            const uint32_t* __restrict__ idx_in,
-                                                            uint32_t* __restrict__ key_out,
-                                                            uint32_t* __restrict__ idx_out, long long M, int shift,
-                                                            int bits, const uint32_t* __restrict__ digit_base,
-                                                            unsigned long long* __restrict__ status,
-                                                            uint32_t* __restrict__ ticket, uint32_t epoch) {
-    __shared__ uint32_t warp_hist[kSortWarps][kRadix + 1];
-    __shared__ uint32_t tile_base[kRadix];
-    __shared__ uint32_t s_tile;
+__global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __restrict__ key_in,
+                                                               const uint32_t* __restrict__ idx_in,
+                                                               uint32_t* __restrict__ key_out,
+                                                               uint32_t* __restrict__ idx_out, long long M, int shift,
+                                                               int bits, const uint32_t* __restrict__ digit_base,
+                                                               unsigned long long* __restrict__ status,
+                                                               uint32_t* __restrict__ ticket, uint32_t epoch) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem& sm = *reinterpret_cast<SortSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < kSortWarps * (kRadix + 1); i += kSortThreads) (&warp_hist[0][0])[i] = 0;
+    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+    for (int i = tid; i < kSortWarps * kRadix; i += kSortThreads) (&sm.warp_cnt[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t tile = s_tile;
-    const long long base = (long long)tile * kSortTile + (long long)warp * (kSortItems * 32) + lane;
+    const uint32_t tile = sm.tile;
+    const long long tile_base = (long long)tile * kSortTile;
+    const long long base = tile_base + (long long)warp * (kSortItems * 32) + lane;
     const uint32_t mask = (1u << bits) - 1u;
 
-    uint32_t k[kSortItems], id[kSortItems], rank[kSortItems];
+    uint32_t k[kSortItems], id[kSortItems];
+    uint16_t rank[kSortItems];
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const long long gidx = base + j * 32;
         const bool valid = gidx < M;
-        k[j] = valid ? key_in[gidx] : 0u;
-        id[j] = kFirst ? (uint32_t)gidx : (valid ? idx_in[gidx] : 0u);
+        k[j] = valid ? __ldg(key_in + gidx) : 0u;
+        id[j] = kFirst ? (uint32_t)gidx : (valid ? __ldg(idx_in + gidx) : 0u);
     }
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const bool valid = (base + j * 32) < M;
-        const uint32_t d = valid ? ((k[j] >> shift) & mask) : (uint32_t)kRadix;
-        const unsigned peers = __match_any_sync(0xffffffffu, d);
-        const int leader = __ffs(peers) - 1;
-        uint32_t c = 0;
-        if (lane == leader) {
-            c = warp_hist[warp][d];
-            warp_hist[warp][d] = c + (uint32_t)__popc(peers);
+        const uint32_t d = (k[j] >> shift) & mask;
+        unsigned peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+        for (int b = 0; b < RICK_RADIX_BITS_MAX; ++b) {
+            if (b < bits) {
+                const bool bit = (d >> b) & 1u;
+                const unsigned bal = __ballot_sync(0xffffffffu, bit);
+                peers &= bit ? bal : ~bal;
+            }
         }
-        c = __shfl_sync(0xffffffffu, c, leader);
-        rank[j] = c + (uint32_t)__popc(peers & lt);
+        const int leader = __ffs(peers) - 1;   // valid lanes always contain themselves
+        uint32_t c = 0;
+        if (valid && lane == leader) {
+            c = sm.warp_cnt[warp][d];
+            sm.warp_cnt[warp][d] = c + (uint32_t)__popc(peers);
+        }
+        c = __shfl_sync(0xffffffffu, c, valid ? leader : lane);
+        rank[j] = (uint16_t)(c + (uint32_t)__popc(peers & lt));
         __syncwarp();
     }
     __syncthreads();
-    if (tid < kRadix) {
+
+    // per-digit totals over the warps (thread t owns digits 2t, 2t+1), exclusive offsets in place
+    uint32_t tot[kDigitsPerThread];
+#pragma unroll
+    for (int q = 0; q < kDigitsPerThread; ++q) {
+        const int d = tid * kDigitsPerThread + q;
         uint32_t running = 0;
 #pragma unroll
         for (int wv = 0; wv < kSortWarps; ++wv) {
-            const uint32_t c = warp_hist[wv][tid];
-            warp_hist[wv][tid] = running;
+            const uint32_t c = sm.warp_cnt[wv][d];
+            sm.warp_cnt[wv][d] = running;
             running += c;
         }
-        unsigned long long* mine = status + (size_t)tile * kRadix + tid;
-        uint32_t excl = 0;
-        if (tile == 0) {
-            st_status(mine, pack_status(2u, epoch, running));
-        } else {
-            st_status(mine, pack_status(1u, epoch, running));
-            long long t = (long long)tile - 1;
-            while (true) {
-                const unsigned long long* pred = status + (size_t)t * kRadix + tid;
-                unsigned long long sv;
-                do {
-                    sv = ld_status(pred);
-                } while ((uint32_t)((sv >> 32) & 0x3FFFFFFFu) != epoch || (sv >> 62) == 0ull);
-                excl += (uint32_t)sv;
-                if ((sv >> 62) == 2ull || t == 0) break;
-                --t;
+        tot[q] = running;
+    }
+    // publish the tile aggregate as early as possible
+    if (tile == 0) {
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q)
+            st_status(status + (size_t)tile * kRadix + tid * kDigitsPerThread + q, pack_status(2u, epoch, tot[q]));
+    } else {
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q)
+            st_status(status + (size_t)tile * kRadix + tid * kDigitsPerThread + q, pack_status(1u, epoch, tot[q]));
+    }
+    // exclusive scan of the digit totals over the tile (slot of each digit in the exchanged order)
+    uint32_t mine = 0;
+#pragma unroll
+    for (int q = 0; q < kDigitsPerThread; ++q) mine += tot[q];
+    uint32_t incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) sm.warp_sum[warp] = incl;
+    __syncthreads();
+    uint32_t before = 0;
+#pragma unroll
+    for (int wv = 0; wv < kSortWarps; ++wv) before += (wv < warp) ? sm.warp_sum[wv] : 0u;
+    uint32_t excl_tile = before + incl - mine;
+    uint32_t texcl[kDigitsPerThread];
+#pragma unroll
+    for (int q = 0; q < kDigitsPerThread; ++q) {
+        texcl[q] = excl_tile;
+        sm.tile_excl[tid * kDigitsPerThread + q] = excl_tile;
+        excl_tile += tot[q];
+    }
+    // decoupled look-back, both digits of the thread in flight together
+    if (tile != 0) {
+        uint32_t excl[kDigitsPerThread];
+        long long t[kDigitsPerThread];
+        bool done[kDigitsPerThread];
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q) { excl[q] = 0; t[q] = (long long)tile - 1; done[q] = false; }
+        bool all_done = false;
+        while (!all_done) {
+            all_done = true;
+#pragma unroll
+            for (int q = 0; q < kDigitsPerThread; ++q) {
+                if (done[q]) continue;
+                const unsigned long long sv = ld_status(status + (size_t)t[q] * kRadix + tid * kDigitsPerThread + q);
+                if ((uint32_t)((sv >> 32) & 0x3FFFFFFFu) == epoch && (sv >> 62) != 0ull) {
+                    excl[q] += (uint32_t)sv;
+                    if ((sv >> 62) == 2ull || t[q] == 0) done[q] = true;
+                    else --t[q];
+                }
+                if (!done[q]) all_done = false;
             }
-            st_status(mine, pack_status(2u, epoch, excl + running));
         }
-        tile_base[tid] = digit_base[tid] + excl;
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q) {
+            const int d = tid * kDigitsPerThread + q;
+            st_status(status + (size_t)tile * kRadix + d, pack_status(2u, epoch, excl[q] + tot[q]));
+            sm.glob[d] = digit_base[d] + excl[q] - texcl[q];
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q) {
+            const int d = tid * kDigitsPerThread + q;
+            sm.glob[d] = digit_base[d] - texcl[q];
+        }
     }
     __syncthreads();
+    // exchange into digit order
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const bool valid = (base + j * 32) < M;
         if (valid) {
             const uint32_t d = (k[j] >> shift) & mask;
-            const uint32_t pos = tile_base[d] + warp_hist[warp][d] + rank[j];
-            key_out[pos] = k[j];
-            idx_out[pos] = id[j];
+            const uint32_t lp = sm.tile_excl[d] + sm.warp_cnt[warp][d] + rank[j];
+            sm.xkey[lp] = k[j];
+            sm.xidx[lp] = id[j];
         }
+    }
+    __syncthreads();
+    const long long left = M - tile_base;
+    const int n_valid = left < (long long)kSortTile ? (int)left : kSortTile;
+    for (int i = tid; i < n_valid; i += kSortThreads) {
+        const uint32_t kk = sm.xkey[i];
+        const uint32_t d = (kk >> shift) & mask;
+        const uint32_t pos = sm.glob[d] + (uint32_t)i;
+        key_out[pos] = kk;
+        idx_out[pos] = sm.xidx[i];
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K3: gather the kept visibilities into sorted SoA arrays
+// K3: gather the kept visibilities into sorted SoA arrays (one 32-B record read per visibility)
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_gather(const long long* __restrict__ n_kept, const uint32_t* __restrict__ idx,
-                                                const float* __restrict__ u, const float* __restrict__ v,
-                                                const float* __restrict__ w, const float2* __restrict__ vis,
-                                                const float* __restrict__ wt, float* __restrict__ u_s,
+                                                const float4* __restrict__ rec, float* __restrict__ u_s,
                                                 float* __restrict__ v_s, float* __restrict__ w_s,
                                                 float2* __restrict__ vis_s, float* __restrict__ wt_s) {
     const long long n = *n_kept;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint32_t src = idx[i];
-        u_s[i] = u[src];
-        v_s[i] = v[src];
-        w_s[i] = w[src];
-        vis_s[i] = vis[src];
-        wt_s[i] = wt[src];
+        const size_t src = (size_t)__ldg(idx + i);
+        const float4 a = __ldg(rec + 2 * src);
+        const float4 b = __ldg(rec + 2 * src + 1);
+        u_s[i] = a.x;
+        v_s[i] = a.y;
+        w_s[i] = a.z;
+        vis_s[i] = make_float2(a.w, b.x);
+        wt_s[i] = b.y;
     }
 }
 
@@ -265,6 +361,14 @@ __global__ void __launch_bounds__(256) k_bin_start(RickGeom g, long long M, cons
 size_t rick_bin_workspace_bytes(const rick_plan* p, long long M) {
     (void)p;
     return carve(nullptr, M).total;
+}
+
+int rick_bin_init() {
+    if (cudaFuncSetAttribute(k_onesweep<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) != cudaSuccess)
+        return RICK_ECUDA;
+    if (cudaFuncSetAttribute(k_onesweep<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) != cudaSuccess)
+        return RICK_ECUDA;
+    return RICK_OK;
 }
 
 int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, const float* w, const float2* vis,
@@ -293,7 +397,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             const long long want = (M + 256 * 8 - 1) / (256 * 8);
             const long long cap = (long long)p->sm_count * 16;
             const int blocks = (int)(want < 1 ? 1 : (want > cap ? cap : want));
-            k_keygen<<<blocks, 256, 0, st>>>(g, M, u, v, w, vis, weight, ws.key_a, key_out, ws.hist,
+            k_keygen<<<blocks, 256, 0, st>>>(g, M, u, v, w, vis, weight, ws.key_a, ws.rec, key_out, ws.hist,
                                              (unsigned long long*)n_kept_dev, lay);
             RICK_LAUNCH_CHECK();
             p->launches++;
@@ -308,11 +412,11 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         uint32_t *kin = ws.key_a, *iin = ws.idx_a, *kout = ws.key_b, *iout = ws.idx_b;
         for (int pass = 0; pass < p->n_pass; ++pass) {
             if (pass == 0)
-                k_onesweep<true><<<n_tiles, kSortThreads, 0, st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
+                k_onesweep<true><<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
                                                                     ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
                                                                     (uint32_t)(pass + 1));
             else
-                k_onesweep<false><<<n_tiles, kSortThreads, 0, st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
+                k_onesweep<false><<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
                                                                      ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
                                                                      (uint32_t)(pass + 1));
             RICK_LAUNCH_CHECK();
@@ -337,8 +441,8 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         {
             const long long want = (M + 255) / 256;
             const long long cap = (long long)p->sm_count * 32;
-            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(n_kept_dev, iin, u, v, w, vis, weight, u_s, v_s, w_s,
-                                                                     vis_s, weight_s);
+            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(n_kept_dev, iin, ws.rec, u_s, v_s, w_s, vis_s,
+                                                                     weight_s);
             RICK_LAUNCH_CHECK();
             p->launches++;
         }

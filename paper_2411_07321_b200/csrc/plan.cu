@@ -88,7 +88,7 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     if (!(dl > 0.0) || !isfinite(dl) || !((double)N * dl < 1.4142135623730951)) return RICK_EINVAL;
     const long long T = N / RICK_TILE;
     const long long n_bins = (long long)Nw * T * T;
-    if (n_bins >= (1ll << 31)) return RICK_EINVAL;
+    if (n_bins > (1ll << 27)) return RICK_EINVAL;   // keeps >= 5 cell bits in the 32-bit sort key [D4']
 
     rick_plan* p = new (std::nothrow) rick_plan();
     if (!p) return RICK_ENOMEM;
@@ -107,14 +107,13 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     // D4': as many in-tile cell bits as fit a 32-bit sort key (10 = the exact cell)
     g.cell_bits = 10;
     while (g.cell_bits > 0 && ((unsigned long long)n_bins << g.cell_bits) > (1ull << 32)) --g.cell_bits;
-    {
-        const unsigned long long s = (unsigned long long)n_bins << g.cell_bits;
-        // n_bins << cb == 2^32: the all-ones key is the last cell of the last tile, which D5 never keeps
-        g.sort_sentinel = s > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)s;
-    }
+    // the largest sort key belongs to row j0 = N-1 of the last tile (cb >= 5 keeps all of j0 & 31),
+    // which D5 never keeps (h >= 1): it is free to mark dropped visibilities and costs no extra key bit
+    g.sort_sentinel = (uint32_t)(((unsigned long long)n_bins << g.cell_bits) - 1ull);
     p->dtype = RICK_C64;
 
-    // radix-sort digit layout: sort keys take values 0 .. sort_sentinel, LSD passes of <= 8 bits
+    if (rick_bin_init() != RICK_OK) { delete p; return RICK_ECUDA; }
+    // radix-sort digit layout: sort keys take values 0 .. sort_sentinel, LSD passes of <= 9 bits
     p->key_bits = ceil_log2_u64((unsigned long long)g.sort_sentinel);
     if (p->key_bits < 1) p->key_bits = 1;
     p->n_pass = (p->key_bits + RICK_RADIX_BITS_MAX - 1) / RICK_RADIX_BITS_MAX;
@@ -178,6 +177,14 @@ int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes
         if (!p->fft_ready) return RICK_ESTATE;
         *fft_bytes = p->fft_work_bytes;
     }
+    return RICK_OK;
+}
+
+int rick_plan_sort_layout(const rick_plan* p, int* key_bits, int* n_pass, int* cell_bits) {
+    if (!p) return RICK_EINVAL;
+    if (key_bits) *key_bits = p->key_bits;
+    if (n_pass) *n_pass = p->n_pass;
+    if (cell_bits) *cell_bits = p->g.cell_bits;
     return RICK_OK;
 }
 

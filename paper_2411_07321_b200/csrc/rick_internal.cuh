@@ -10,7 +10,7 @@
 
 #define RICK_TILE 32          // uv tile edge of the sort key (BASELINE.json north_star (2))
 #define RICK_MAX_PASSES 4
-#define RICK_RADIX_BITS_MAX 8
+#define RICK_RADIX_BITS_MAX 9
 
 // Geometry constants handed to kernels by value.
 struct RickGeom {
@@ -24,7 +24,7 @@ struct RickGeom {
     double sigma;
     uint32_t n_bins; // Nw * T * T, also the sentinel tile key [D4]
     int cell_bits;   // cb: in-tile cell bits appended to the tile key in the sort key [D4']
-    uint32_t sort_sentinel;  // sort key of a dropped visibility: min(n_bins << cb, 2^32 - 1)
+    uint32_t sort_sentinel;  // sort key of a dropped visibility: (n_bins << cb) - 1, a key D5 never keeps
     double tap_c;    // 1 / (2 sigma^2)
 };
 
@@ -121,5 +121,6 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
                   unsigned long long* bin_start_out, void* workspace, size_t workspace_bytes,
                   long long* n_kept_dev, cudaStream_t st);
 size_t rick_bin_workspace_bytes(const rick_plan* p, long long M);
+int rick_bin_init();   // one-time kernel attributes (dynamic shared memory opt-in)
 int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st);
 int rick_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);

@@ -127,14 +127,14 @@ def test_stable_sort_three_ways():
 
 def test_sort_key_refines_tile_key():
     """D4': hand values, the refinement property (same grouping by tile, cells adjacent inside a tile)
-    and the sentinel, for a plan where all 10 cell bits fit and one (Nw T^2 = 2^22) where only... they
-    exactly fill 32 bits, plus one (Nw T^2 = 2^23) that keeps 9 bits."""
+    and the sentinel, for plans where all 10 cell bits fit (Nw T^2 = 2^22 fills the 32 bits exactly),
+    one that keeps 9 bits (2^23) and one that keeps 6 (2^26)."""
     # hand case: N=256 (T=8), Nw=8 -> n_bins=512, cb=10; vis at i0=131, j0=37, k=3:
     # key=(3*8+1)*8+4=204, cell=(37&31)*32+(131&31)=5*32+3=163 -> 204*1024+163
     plan = O.Plan(N=256, Nw=8, support=7, sigma=1.0, w_min=0.0, w_max=8.0, dl=0.2 / 256)
     key = np.array([204, 512, 0], np.uint32)
     sk, cb = O.sort_key(plan, key, np.array([131, -1, 3], np.int32), np.array([37, -1, 3], np.int32))
-    assert cb == 10 and list(sk) == [204 * 1024 + 163, 512 * 1024, 3 * 32 + 3]
+    assert cb == 10 and list(sk) == [204 * 1024 + 163, 512 * 1024 - 1, 3 * 32 + 3]
     rng = np.random.default_rng(3)
     for N, Nw, ecb in ((512, 16, 10), (16384, 16, 10), (16384, 32, 9), (32768, 64, 6)):
         plan = O.Plan(N=N, Nw=Nw, support=9, sigma=1.3, w_min=-50.0, w_max=50.0, dl=0.5 / N)
@@ -152,8 +152,7 @@ def test_sort_key_refines_tile_key():
         assert cb == ecb
         kept = key < plan.n_bins
         assert kept[-1] and 0 < n_kept < M
-        top = plan.n_bins << cb
-        assert np.all(sk[~kept] == min(top, 2**32 - 1)) and np.all(sk[kept].astype(np.int64) < sk[~kept][0])
+        assert np.all(sk[~kept] == (plan.n_bins << cb) - 1) and np.all(sk[kept].astype(np.int64) < sk[~kept][0])
         assert np.array_equal(sk[kept] >> cb, key[kept])                      # refinement of the tile key
         cell = ((j0[kept] & 31) << 5) | (i0[kept] & 31)
         assert np.array_equal(sk[kept] & ((1 << cb) - 1), cell >> (10 - cb))
