@@ -19,7 +19,6 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kSortWarps = kSortThreads / 32;
-constexpr int kDigitsPerThread = kRadix / kSortThreads;   // 2
 
 struct SortLayout {
     int n_pass;
@@ -163,12 +162,12 @@ struct SortSmem {
     uint32_t tile;
 };
 
-template <bool kFirst>
+template <bool kFirst, int kBits>
 __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __restrict__ key_in,
                                                                const uint32_t* __restrict__ idx_in,
                                                                uint32_t* __restrict__ key_out,
                                                                uint32_t* __restrict__ idx_out, long long M, int shift,
-                                                               int bits, const uint32_t* __restrict__ digit_base,
+                                                               const uint32_t* __restrict__ digit_base,
                                                                unsigned long long* __restrict__ status,
                                                                uint32_t* __restrict__ ticket, uint32_t epoch) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -180,7 +179,9 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __
     const uint32_t tile = sm.tile;
     const long long tile_base = (long long)tile * kSortTile;
     const long long base = tile_base + (long long)warp * (kSortItems * 32) + lane;
-    const uint32_t mask = (1u << bits) - 1u;
+    constexpr uint32_t mask = (1u << kBits) - 1u;
+    constexpr int kDigitsPerThread = (1 << kBits) / kSortThreads;   // 2 (9-bit digits) or 1 (8-bit digits)
+    static_assert(kDigitsPerThread >= 1, "digit width too small for the block size");
 
     uint32_t k[kSortItems], id[kSortItems];
     uint16_t rank[kSortItems];
@@ -198,12 +199,10 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __
         const uint32_t d = (k[j] >> shift) & mask;
         unsigned peers = __ballot_sync(0xffffffffu, valid);
 #pragma unroll
-        for (int b = 0; b < RICK_RADIX_BITS_MAX; ++b) {
-            if (b < bits) {
-                const bool bit = (d >> b) & 1u;
-                const unsigned bal = __ballot_sync(0xffffffffu, bit);
-                peers &= bit ? bal : ~bal;
-            }
+        for (int b = 0; b < kBits; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const unsigned bal = __ballot_sync(0xffffffffu, bit);
+            peers &= bit ? bal : ~bal;
         }
         const int leader = __ffs(peers) - 1;   // valid lanes always contain themselves
         uint32_t c = 0;
@@ -264,33 +263,35 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __
         sm.tile_excl[tid * kDigitsPerThread + q] = excl_tile;
         excl_tile += tot[q];
     }
-    // decoupled look-back, both digits of the thread in flight together
+    // decoupled look-back: a window of kLookWin predecessors per digit is loaded at once (independent
+    // loads in flight), then consumed from the nearest tile backwards up to the first inclusive prefix
     if (tile != 0) {
-        uint32_t excl[kDigitsPerThread];
-        long long t[kDigitsPerThread];
-        bool done[kDigitsPerThread];
-#pragma unroll
-        for (int q = 0; q < kDigitsPerThread; ++q) { excl[q] = 0; t[q] = (long long)tile - 1; done[q] = false; }
-        bool all_done = false;
-        while (!all_done) {
-            all_done = true;
-#pragma unroll
-            for (int q = 0; q < kDigitsPerThread; ++q) {
-                if (done[q]) continue;
-                const unsigned long long sv = ld_status(status + (size_t)t[q] * kRadix + tid * kDigitsPerThread + q);
-                if ((uint32_t)((sv >> 32) & 0x3FFFFFFFu) == epoch && (sv >> 62) != 0ull) {
-                    excl[q] += (uint32_t)sv;
-                    if ((sv >> 62) == 2ull || t[q] == 0) done[q] = true;
-                    else --t[q];
-                }
-                if (!done[q]) all_done = false;
-            }
-        }
+        constexpr int kLookWin = 4;
 #pragma unroll
         for (int q = 0; q < kDigitsPerThread; ++q) {
             const int d = tid * kDigitsPerThread + q;
-            st_status(status + (size_t)tile * kRadix + d, pack_status(2u, epoch, excl[q] + tot[q]));
-            sm.glob[d] = digit_base[d] + excl[q] - texcl[q];
+            uint32_t excl = 0;
+            long long t = (long long)tile - 1;
+            bool done = false;
+            while (!done) {
+                unsigned long long sv[kLookWin];
+#pragma unroll
+                for (int x = 0; x < kLookWin; ++x) {
+                    const long long tt = t - x;
+                    sv[x] = tt >= 0 ? ld_status(status + (size_t)tt * kRadix + d) : 0ull;
+                }
+#pragma unroll
+                for (int x = 0; x < kLookWin; ++x) {
+                    if (done || t < 0) continue;
+                    const bool ready = (uint32_t)((sv[x] >> 32) & 0x3FFFFFFFu) == epoch && (sv[x] >> 62) != 0ull;
+                    if (!ready) break;           // re-poll from this tile
+                    excl += (uint32_t)sv[x];
+                    if ((sv[x] >> 62) == 2ull || t == 0) done = true;
+                    --t;
+                }
+            }
+            st_status(status + (size_t)tile * kRadix + d, pack_status(2u, epoch, excl + tot[q]));
+            sm.glob[d] = digit_base[d] + excl - texcl[q];
         }
     } else {
 #pragma unroll
@@ -364,9 +365,12 @@ size_t rick_bin_workspace_bytes(const rick_plan* p, long long M) {
 }
 
 int rick_bin_init() {
-    if (cudaFuncSetAttribute(k_onesweep<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) != cudaSuccess)
-        return RICK_ECUDA;
-    if (cudaFuncSetAttribute(k_onesweep<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) != cudaSuccess)
+    const int bytes = (int)sizeof(SortSmem);
+    const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    if (cudaFuncSetAttribute(k_onesweep<true, 8>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9>, a, bytes) != cudaSuccess)
         return RICK_ECUDA;
     return RICK_OK;
 }
@@ -411,14 +415,13 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         const unsigned n_tiles = (unsigned)((M + kSortTile - 1) / kSortTile);
         uint32_t *kin = ws.key_a, *iin = ws.idx_a, *kout = ws.key_b, *iout = ws.idx_b;
         for (int pass = 0; pass < p->n_pass; ++pass) {
-            if (pass == 0)
-                k_onesweep<true><<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
-                                                                    ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
-                                                                    (uint32_t)(pass + 1));
-            else
-                k_onesweep<false><<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass], lay.bits[pass],
-                                                                     ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
-                                                                     (uint32_t)(pass + 1));
+            const bool first = (pass == 0);
+            const bool nine = (lay.bits[pass] == 9);
+            auto kern = first ? (nine ? k_onesweep<true, 9> : k_onesweep<true, 8>)
+                              : (nine ? k_onesweep<false, 9> : k_onesweep<false, 8>);
+            kern<<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
+                                                                 ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
+                                                                 (uint32_t)(pass + 1));
             RICK_LAUNCH_CHECK();
             p->launches++;
             uint32_t* t;

@@ -116,14 +116,14 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     // radix-sort digit layout: sort keys take values 0 .. sort_sentinel, LSD passes of <= 9 bits
     p->key_bits = ceil_log2_u64((unsigned long long)g.sort_sentinel);
     if (p->key_bits < 1) p->key_bits = 1;
-    p->n_pass = (p->key_bits + RICK_RADIX_BITS_MAX - 1) / RICK_RADIX_BITS_MAX;
+    // digits are 9 bits wide (up to 27 key bits: 1-3 passes) or 8 bits wide (28-32 key bits: 4 passes);
+    // the top digit may extend past the key (those bits are zero)
     {
-        int shift = 0;
+        const int width = p->key_bits <= 27 ? 9 : 8;
+        p->n_pass = (p->key_bits + width - 1) / width;
         for (int i = 0; i < p->n_pass; ++i) {
-            int bits = p->key_bits / p->n_pass + (i < (p->key_bits % p->n_pass) ? 1 : 0);
-            p->digit_bits[i] = bits;
-            p->digit_shift[i] = shift;
-            shift += bits;
+            p->digit_bits[i] = width;
+            p->digit_shift[i] = i * width;
         }
     }
 
