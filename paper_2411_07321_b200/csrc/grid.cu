@@ -14,8 +14,8 @@
 // shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on sm_100a), and the number
 // of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to kRunItems).
 //
-// The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) depends only on the target cell and
-// is applied once at the flush.
+// The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) costs nothing: (-1)^(a+b) is folded
+// into the taps as compile-time negations and (-1)^(i0+j0) into the sign of the weight.
 #include "rick_internal.cuh"
 
 namespace {
@@ -25,6 +25,7 @@ constexpr int kRunItems = 16;   // consecutive sorted visibilities per thread (a
 
 struct TapConst {
     double K[8];   // K[t] = exp(-t^2 / (2 sigma^2)), t = 0 .. h
+    float Kf[8];   // the same, rounded to fp32
 };
 
 __device__ __forceinline__ void red_add_cell(float2* addr, float re, float im) {
@@ -41,35 +42,50 @@ __device__ __forceinline__ float ex2_approx(float x) {
     return y;
 }
 
-// Taps of one axis, t[a] = g(d0 + a - h), a = 0 .. S-1, d0 = i0 - x (formed in fp64, narrowed once).
-// fp32: one MUFU.EX2 per tap.
+// Taps of one axis with the alternating sign of the modulated mesh folded in:
+//     t[a] = (-1)^a g(d0 + a - h),  a = 0 .. S-1,  d0 = i0 - x (formed in fp64, narrowed once),
+// through the exact identity g(d0 + s) = g(d0) E^s g(s), E = exp(-d0 / sigma^2): three exponentials per
+// axis instead of S (fp32: MUFU.EX2; fp64: two exp and one reciprocal).  The (-1)^a are compile-time
+// negations (operand modifiers); the remaining run-constant factor (-1)^(i0+j0) multiplies weight * V.
 template <int S>
-__device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst&) {
+__device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst& tc) {
     constexpr int h = (S - 1) / 2;
     const float c2 = (float)(-g.tap_c * 1.4426950408889634);   // -log2(e) / (2 sigma^2)
     const float d = (float)d0;
+    const float g0 = ex2_approx(d * d * c2);
+    const float e = 2.0f * d * c2;
+    const float E = ex2_approx(e), Ei = ex2_approx(-e);
+    float pp = g0, pm = g0;
+    t[h] = (h & 1) ? -g0 : g0;
 #pragma unroll
-    for (int a = 0; a < S; ++a) {
-        const float da = d + (float)(a - h);
-        t[a] = ex2_approx(da * da * c2);
+    for (int s = 1; s <= h; ++s) {
+        pp *= E;
+        pm *= Ei;
+        const float a = pp * tc.Kf[s], b = pm * tc.Kf[s];
+        t[h + s] = ((h + s) & 1) ? -a : a;
+        t[h - s] = ((h - s) & 1) ? -b : b;
     }
 }
-// fp64: g(d0 + s) = g(d0) E^s K[|s|] with E = exp(-d0 / sigma^2): two exp and one reciprocal per axis.
 template <int S>
 __device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, const TapConst& tc) {
     constexpr int h = (S - 1) / 2;
     const double g0 = exp(-d0 * d0 * g.tap_c);
     const double E = exp(-2.0 * d0 * g.tap_c);
     const double Ei = 1.0 / E;
-    t[h] = g0;
+    t[h] = (h & 1) ? -g0 : g0;
     double pp = g0, pm = g0;
 #pragma unroll
     for (int s = 1; s <= h; ++s) {
         pp *= E;
         pm *= Ei;
-        t[h + s] = pp * tc.K[s];
-        t[h - s] = pm * tc.K[s];
+        const double a = pp * tc.K[s], b = pm * tc.K[s];
+        t[h + s] = ((h + s) & 1) ? -a : a;
+        t[h - s] = ((h - s) & 1) ? -b : b;
     }
+}
+
+__device__ __forceinline__ void prefetch_l1(const void* p) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
 
 template <typename real> struct CellOf;
@@ -99,6 +115,16 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
     const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * kRunItems;
     if (first >= n) return;
     const size_t N = (size_t)g.N;
+    // pull the thread's twelve 32-B sectors into L1 before the first use (the loads below then hit)
+#pragma unroll
+    for (int q = 0; q < kRunItems / 8; ++q) {
+        prefetch_l1(u_s + first + 8 * q);
+        prefetch_l1(v_s + first + 8 * q);
+        prefetch_l1(w_s + first + 8 * q);
+        prefetch_l1(wt_s + first + 8 * q);
+        prefetch_l1(vis_s + first + 8 * q);
+        prefetch_l1(vis_s + first + 8 * q + 4);
+    }
 
 #pragma unroll
     for (int pass = 0; pass < kPasses; ++pass) {
@@ -114,14 +140,12 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
 
         auto flush = [&]() {
             cell* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)(ci - h);
-            const real s0 = ((ci + cj) & 1) ? (real)-1 : (real)1;
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
 #pragma unroll
                     for (int a = 0; a < S; ++a) {
-                        const real sg = ((a + b0 + r) & 1) ? -s0 : s0;
-                        red_add_cell(base + (size_t)r * N + a, ar[r][a] * sg, ai[r][a] * sg);
+                        red_add_cell(base + (size_t)r * N + a, ar[r][a], ai[r][a]);
                         ar[r][a] = ai[r][a] = (real)0;
                     }
                 }
@@ -137,7 +161,8 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
             real gx[S], gy[S];
             taps<S>(gx, (double)loc.i0 - loc.x, g, tc);
             taps<S>(gy, (double)loc.j0 - loc.y, g, tc);
-            const real vr = (real)wgt * (real)re, vi = (real)wgt * (real)im;
+            const real ws = ((loc.i0 + loc.j0) & 1) ? -(real)wgt : (real)wgt;   // (-1)^(i0+j0) weight
+            const real vr = ws * (real)re, vi = ws * (real)im;
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
@@ -171,7 +196,10 @@ template <typename real, int S, int RB>
 void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
     typedef typename CellOf<real>::type cell;
     TapConst tc;
-    for (int t = 0; t < 8; ++t) tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
+    for (int t = 0; t < 8; ++t) {
+        tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
+        tc.Kf[t] = (float)tc.K[t];
+    }
     const long long per_block = (long long)kRunThreads * kRunItems;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
     k_grid_runs<real, S, RB><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
