@@ -9,7 +9,7 @@
 //     acc[b][a] += gx[a] * (gy[b] * weight * V)          2 FMAs per cell and visibility
 //
 // and only when the nearest cell changes (or its range ends) adds the footprint to the mesh with
-// vector reductions in L2 (red.global.add.v2.f32 / red.global.add.f64).  Lanes of a warp hold
+// vector reductions in L2 (red.global.add.v4.f32, two cells each / red.global.add.f64).  Lanes of a warp hold
 // neighbouring cells, so those reductions fall into the same few sectors.  No shared memory, no
 // shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on sm_100a), and the number
 // of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to kRunItems).
@@ -21,7 +21,10 @@
 namespace {
 
 constexpr int kRunThreads = 128;
-constexpr int kRunItems = 16;   // consecutive sorted visibilities per thread (a multiple of 4)
+#ifndef RICK_RUN_ITEMS
+#define RICK_RUN_ITEMS 32
+#endif
+constexpr int kRunItems = RICK_RUN_ITEMS;   // consecutive sorted visibilities per thread (a multiple of 8)
 
 struct TapConst {
     double K[8];   // K[t] = exp(-t^2 / (2 sigma^2)), t = 0 .. h
@@ -36,6 +39,11 @@ __device__ __forceinline__ void red_add_cell(double2* addr, double re, double im
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"((double*)addr + 1), "d"(im) : "memory");
 }
 
+__device__ __forceinline__ void red_add_pair(float2* addr, float re0, float im0, float re1, float im1) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(re0), "f"(im0), "f"(re1), "f"(im1)
+                 : "memory");
+}
+
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -47,7 +55,7 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // through the exact identity g(d0 + s) = g(d0) E^s g(s), E = exp(-d0 / sigma^2): three exponentials per
 // axis instead of S (fp32: MUFU.EX2; fp64: two exp and one reciprocal).  The (-1)^a are compile-time
 // negations (operand modifiers); the remaining run-constant factor (-1)^(i0+j0) multiplies weight * V.
-template <int S>
+template <int S, bool kSigned>
 __device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst& tc) {
     constexpr int h = (S - 1) / 2;
     const float c2 = (float)(-g.tap_c * 1.4426950408889634);   // -log2(e) / (2 sigma^2)
@@ -56,31 +64,31 @@ __device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, con
     const float e = 2.0f * d * c2;
     const float E = ex2_approx(e), Ei = ex2_approx(-e);
     float pp = g0, pm = g0;
-    t[h] = (h & 1) ? -g0 : g0;
+    t[h] = (kSigned && (h & 1)) ? -g0 : g0;
 #pragma unroll
     for (int s = 1; s <= h; ++s) {
         pp *= E;
         pm *= Ei;
         const float a = pp * tc.Kf[s], b = pm * tc.Kf[s];
-        t[h + s] = ((h + s) & 1) ? -a : a;
-        t[h - s] = ((h - s) & 1) ? -b : b;
+        t[h + s] = (kSigned && ((h + s) & 1)) ? -a : a;
+        t[h - s] = (kSigned && ((h - s) & 1)) ? -b : b;
     }
 }
-template <int S>
+template <int S, bool kSigned>
 __device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, const TapConst& tc) {
     constexpr int h = (S - 1) / 2;
     const double g0 = exp(-d0 * d0 * g.tap_c);
     const double E = exp(-2.0 * d0 * g.tap_c);
     const double Ei = 1.0 / E;
-    t[h] = (h & 1) ? -g0 : g0;
+    t[h] = (kSigned && (h & 1)) ? -g0 : g0;
     double pp = g0, pm = g0;
 #pragma unroll
     for (int s = 1; s <= h; ++s) {
         pp *= E;
         pm *= Ei;
         const double a = pp * tc.K[s], b = pm * tc.K[s];
-        t[h + s] = ((h + s) & 1) ? -a : a;
-        t[h - s] = ((h - s) & 1) ? -b : b;
+        t[h + s] = (kSigned && ((h + s) & 1)) ? -a : a;
+        t[h - s] = (kSigned && ((h - s) & 1)) ? -b : b;
     }
 }
 
@@ -102,7 +110,7 @@ __device__ __forceinline__ float4 load4(const float* __restrict__ a, long long p
     return r;
 }
 
-template <typename real, int S, int RB>
+template <typename real, int S, int RB, int L>
 __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                           const float* __restrict__ u_s, const float* __restrict__ v_s,
                                                           const float* __restrict__ w_s, const float2* __restrict__ vis_s,
@@ -111,13 +119,17 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
     typedef typename CellOf<real>::type cell;
     constexpr int h = (S - 1) / 2;
     constexpr int kPasses = (S + RB - 1) / RB;
+    // fp32: the footprint columns live in an even-aligned window of W = S + 1 cells, so that every pair of
+    // cells is one 16-byte red.global.add.v4.f32 (the extra column carries a zero tap); fp64: W = S.
+    constexpr bool kWin = (sizeof(real) == 4);
+    constexpr int W = kWin ? S + 1 : S;
     const long long n = *n_kept;
-    const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * kRunItems;
+    const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * L;
     if (first >= n) return;
     const size_t N = (size_t)g.N;
-    // pull the thread's twelve 32-B sectors into L1 before the first use (the loads below then hit)
+    // pull the thread's 32-B sectors into L1 before the first use (the loads below then hit)
 #pragma unroll
-    for (int q = 0; q < kRunItems / 8; ++q) {
+    for (int q = 0; q < L / 8; ++q) {
         prefetch_l1(u_s + first + 8 * q);
         prefetch_l1(v_s + first + 8 * q);
         prefetch_l1(w_s + first + 8 * q);
@@ -128,25 +140,37 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
 
 #pragma unroll
     for (int pass = 0; pass < kPasses; ++pass) {
-        constexpr int dummy = 0;
-        (void)dummy;
         const int b0 = pass * RB;
-        real ar[RB][S], ai[RB][S];
+        real ar[RB][W], ai[RB][W];
 #pragma unroll
         for (int r = 0; r < RB; ++r)
 #pragma unroll
-            for (int a = 0; a < S; ++a) ar[r][a] = ai[r][a] = (real)0;
+            for (int a = 0; a < W; ++a) ar[r][a] = ai[r][a] = (real)0;
         int ci = -1, cj = 0, ck = 0;
 
         auto flush = [&]() {
-            cell* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)(ci - h);
+            const int iw = kWin ? ((ci - h) & ~1) : (ci - h);   // first column of the window
+            cell* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)iw;
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
+                    if constexpr (kWin) {
 #pragma unroll
-                    for (int a = 0; a < S; ++a) {
-                        red_add_cell(base + (size_t)r * N + a, ar[r][a], ai[r][a]);
-                        ar[r][a] = ai[r][a] = (real)0;
+                        for (int a = 0; a < W; a += 2) {
+                            float2* dst = (float2*)(base + (size_t)r * N + a);
+                            // the zero column may fall past the end of the row (only when i0 = N-1-h)
+                            if (a + 2 == W && iw + W > (int)N)
+                                red_add_cell(dst, (float)ar[r][a], (float)ai[r][a]);
+                            else
+                                red_add_pair(dst, (float)ar[r][a], (float)ai[r][a], (float)ar[r][a + 1], (float)ai[r][a + 1]);
+                            ar[r][a] = ai[r][a] = ar[r][a + 1] = ai[r][a + 1] = (real)0;
+                        }
+                    } else {
+#pragma unroll
+                        for (int a = 0; a < W; ++a) {
+                            red_add_cell(base + (size_t)r * N + a, ar[r][a], ai[r][a]);
+                            ar[r][a] = ai[r][a] = (real)0;
+                        }
                     }
                 }
             }
@@ -158,17 +182,33 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
                 if (ci >= 0) flush();
                 ci = loc.i0; cj = loc.j0; ck = loc.k;
             }
-            real gx[S], gy[S];
-            taps<S>(gx, (double)loc.i0 - loc.x, g, tc);
-            taps<S>(gy, (double)loc.j0 - loc.y, g, tc);
-            const real ws = ((loc.i0 + loc.j0) & 1) ? -(real)wgt : (real)wgt;   // (-1)^(i0+j0) weight
+            real gx[W], gy[S];
+            taps<S, true>(gy, (double)loc.j0 - loc.y, g, tc);
+            bool neg;
+            if constexpr (kWin) {
+                // window column c <-> cell iw + c, iw even: sign (-1)^c at compile time; tap index c - o
+                real t[S];
+                taps<S, false>(t, (double)loc.i0 - loc.x, g, tc);
+                const bool o = ((loc.i0 - h) & 1) != 0;
+#pragma unroll
+                for (int c = 0; c < W; ++c) {
+                    const real lo = (c >= 1) ? t[c - 1] : (real)0, hi = (c < S) ? t[c] : (real)0;
+                    const real v = o ? lo : hi;
+                    gx[c] = (c & 1) ? -v : v;
+                }
+                neg = ((loc.j0 - h) & 1) != 0;            // (-1)^(j0-h): the rest of (-1)^(i+j)
+            } else {
+                taps<S, true>(gx, (double)loc.i0 - loc.x, g, tc);
+                neg = ((loc.i0 + loc.j0) & 1) != 0;       // (-1)^(i0+j0)
+            }
+            const real ws = neg ? -(real)wgt : (real)wgt;
             const real vr = ws * (real)re, vi = ws * (real)im;
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
                     const real yr = gy[b0 + r] * vr, yi = gy[b0 + r] * vi;
 #pragma unroll
-                    for (int a = 0; a < S; ++a) {
+                    for (int a = 0; a < W; ++a) {
                         ar[r][a] = fma(gx[a], yr, ar[r][a]);
                         ai[r][a] = fma(gx[a], yi, ai[r][a]);
                     }
@@ -177,7 +217,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
         };
 
 #pragma unroll 1
-        for (int i = 0; i < kRunItems; i += 4) {
+        for (int i = 0; i < L; i += 4) {
             const long long p = first + i;
             if (p >= n) break;
             const float4 u4 = load4(u_s, p, n), v4 = load4(v_s, p, n), w4 = load4(w_s, p, n), t4 = load4(wt_s, p, n);
@@ -202,7 +242,7 @@ void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
     }
     const long long per_block = (long long)kRunThreads * kRunItems;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
-    k_grid_runs<real, S, RB><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
+    k_grid_runs<real, S, RB, kRunItems><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
                                                               (const float2*)p->vis_s, p->weight_s, (cell*)grid);
 }
 
