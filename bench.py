@@ -283,23 +283,26 @@ def main():
                 "launch_ms": launch_ms, "alg_bytes_per_launch": launch_bytes}
 
     # end to end through rick_image_from_host: pinned host inputs -> host image, copies inside the region
-    host = [x.cpu().pin_memory() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
-    out = torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory()
-    im.run_from_host(*host, out)
-    torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.e2e_steps):
+    host = [x.cpu() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
+    e2e = None
+    if args.e2e_steps > 0:
+        host = [x.pin_memory() for x in host]
+        out = torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory()
         im.run_from_host(*host, out)
-    torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e = {"value": world * M / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
-           "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps}
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            im.run_from_host(*host, out)
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / args.e2e_steps
+        if dist is not None:
+            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        e2e = {"value": world * M / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
+               "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps}
 
     if rank != 0:
         if dist is not None:
