@@ -29,6 +29,7 @@ struct SortLayout {
 struct Workspace {
     uint32_t *key_a, *key_b, *idx_a, *idx_b;
     float4* rec;                     // [M][2]: (u, v, w, re), (im, weight, -, -): one 32-B sector per visibility
+    float2 *grec_b, *grec_c;         // gridder records b[], c[] of the sorted kept visibilities (rick_internal.cuh)
     uint32_t* hist;                  // [RICK_MAX_PASSES][kRadix] digit counts -> exclusive bases
     uint32_t* ticket;                // [RICK_MAX_PASSES] dynamic tile ids
     unsigned long long* status;      // [n_tiles][kRadix] look-back words
@@ -42,11 +43,16 @@ Workspace carve(void* base, long long M) {
     const size_t n_tiles = (m + kSortTile - 1) / kSortTile;
     size_t off = 0;
     char* b = (char*)base;
-    ws.key_a = (uint32_t*)(b + off); off += rick_align256(4 * m);
-    ws.key_b = (uint32_t*)(b + off); off += rick_align256(4 * m);
-    ws.idx_a = (uint32_t*)(b + off); off += rick_align256(4 * m);
-    ws.idx_b = (uint32_t*)(b + off); off += rick_align256(4 * m);
+    const size_t mp = (m + RICK_GREC_PAD - 1) / RICK_GREC_PAD * RICK_GREC_PAD;   // whole gridder chunks
+    // (key, index) ping and pong, each pair contiguous: the pair that is dead after the last pass is
+    // reused for the 8-byte gridder records a[]
+    ws.key_a = (uint32_t*)(b + off); off += 4 * mp;
+    ws.idx_a = (uint32_t*)(b + off); off += 4 * mp;
+    ws.key_b = (uint32_t*)(b + off); off += 4 * mp;
+    ws.idx_b = (uint32_t*)(b + off); off += 4 * mp;
     ws.rec = (float4*)(b + off); off += rick_align256(32 * m);
+    ws.grec_b = (float2*)(b + off); off += rick_align256(8 * mp);
+    ws.grec_c = (float2*)(b + off); off += rick_align256(8 * mp);
     ws.zero_offset = off;
     ws.hist = (uint32_t*)(b + off); off += rick_align256(sizeof(uint32_t) * RICK_MAX_PASSES * kRadix);
     ws.ticket = (uint32_t*)(b + off); off += rick_align256(sizeof(uint32_t) * RICK_MAX_PASSES);
@@ -325,12 +331,17 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __
 }
 
 // ---------------------------------------------------------------------------------------------
-// K3: gather the kept visibilities into sorted SoA arrays (one 32-B record read per visibility)
+// K3: gather the kept visibilities into sorted SoA arrays (one 32-B record read per visibility) and
+// write the gridder records: nearest cell, plane, fractional offsets (fp64 difference narrowed once)
+// and weight * V with the run-constant checkerboard factor (-1)^(j0-h) of the fp32 gridder folded in.
+// The kernel waits on memory, so the fp64 coordinate arithmetic is free here.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_gather(const long long* __restrict__ n_kept, const uint32_t* __restrict__ idx,
-                                                const float4* __restrict__ rec, float* __restrict__ u_s,
-                                                float* __restrict__ v_s, float* __restrict__ w_s,
-                                                float2* __restrict__ vis_s, float* __restrict__ wt_s) {
+__global__ void __launch_bounds__(256) k_gather(RickGeom g, const long long* __restrict__ n_kept,
+                                                const uint32_t* __restrict__ idx, const float4* __restrict__ rec,
+                                                float* __restrict__ u_s, float* __restrict__ v_s,
+                                                float* __restrict__ w_s, float2* __restrict__ vis_s,
+                                                float* __restrict__ wt_s, uint2* __restrict__ ga,
+                                                float2* __restrict__ gb, float2* __restrict__ gc) {
     const long long n = *n_kept;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
@@ -342,6 +353,11 @@ __global__ void __launch_bounds__(256) k_gather(const long long* __restrict__ n_
         w_s[i] = a.z;
         vis_s[i] = make_float2(a.w, b.x);
         wt_s[i] = b.y;
+        const RickLoc r = rick_locate(g, a.x, a.y, a.z);
+        const float ws = ((r.j0 - g.h) & 1) ? -b.y : b.y;
+        ga[i] = make_uint2((uint32_t)r.i0 | ((uint32_t)r.j0 << 16), (uint32_t)r.k);
+        gb[i] = make_float2((float)((double)r.i0 - r.x), (float)((double)r.j0 - r.y));
+        gc[i] = make_float2(ws * a.w, ws * b.x);
     }
 }
 
@@ -414,6 +430,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
 
         const unsigned n_tiles = (unsigned)((M + kSortTile - 1) / kSortTile);
         uint32_t *kin = ws.key_a, *iin = ws.idx_a, *kout = ws.key_b, *iout = ws.idx_b;
+        (void)iout;
         for (int pass = 0; pass < p->n_pass; ++pass) {
             const bool first = (pass == 0);
             const bool nine = (lay.bits[pass] == 9);
@@ -444,16 +461,18 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         {
             const long long want = (M + 255) / 256;
             const long long cap = (long long)p->sm_count * 32;
-            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(n_kept_dev, iin, ws.rec, u_s, v_s, w_s, vis_s,
-                                                                     weight_s);
+            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, n_kept_dev, iin, ws.rec, u_s, v_s, w_s, vis_s,
+                                                                     weight_s, (uint2*)kout, ws.grec_b, ws.grec_c);
             RICK_LAUNCH_CHECK();
             p->launches++;
+            p->grec_a = (const uint2*)kout;
         }
         rick_stage_end(p, RICK_T_GATHER, st);
     }
     p->M = M;
     p->u_s = u_s; p->v_s = v_s; p->w_s = w_s; p->vis_s = vis_s; p->weight_s = weight_s;
     p->n_kept_dev = n_kept_dev;
+    p->grec_b = ws.grec_b; p->grec_c = ws.grec_c;
     p->bound = true;
     return RICK_OK;
 }

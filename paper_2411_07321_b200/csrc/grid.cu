@@ -56,10 +56,8 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // axis instead of S (fp32: MUFU.EX2; fp64: two exp and one reciprocal).  The (-1)^a are compile-time
 // negations (operand modifiers); the remaining run-constant factor (-1)^(i0+j0) multiplies weight * V.
 template <int S, bool kSigned>
-__device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst& tc) {
+__device__ __forceinline__ void taps_f32(float* t, float d, float c2, const TapConst& tc) {
     constexpr int h = (S - 1) / 2;
-    const float c2 = (float)(-g.tap_c * 1.4426950408889634);   // -log2(e) / (2 sigma^2)
-    const float d = (float)d0;
     const float g0 = ex2_approx(d * d * c2);
     const float e = 2.0f * d * c2;
     const float E = ex2_approx(e), Ei = ex2_approx(-e);
@@ -73,6 +71,10 @@ __device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, con
         t[h + s] = (kSigned && ((h + s) & 1)) ? -a : a;
         t[h - s] = (kSigned && ((h - s) & 1)) ? -b : b;
     }
+}
+template <int S, bool kSigned>
+__device__ __forceinline__ void taps(float* t, double d0, const RickGeom& g, const TapConst& tc) {
+    taps_f32<S, kSigned>(t, (float)d0, (float)(-g.tap_c * 1.4426950408889634), tc);   // c2 = -log2(e) / (2 sigma^2)
 }
 template <int S, bool kSigned>
 __device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, const TapConst& tc) {
@@ -232,6 +234,151 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// fp32 mesh: the record-fed gridder.  A CTA stages its 128 x L gridder records (rick_bin's gather wrote
+// them: cell, plane, fractional offsets, signed weight * V; 24 B per visibility in three 8-byte streams)
+// into shared memory with coalesced 16-byte cp.async copies, every byte of HBM read exactly once and all
+// copies of a CTA in flight together; the second CTA of the SM computes meanwhile.  The 16-byte pieces
+// are XOR-swizzled so that the per-thread reads (thread t owns records t*L .. t*L+L-1: that is what
+// makes runs) are bank-conflict free.  No fp64 and no global loads inside the accumulation loop.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+template <int S, int RB, int L>
+__global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
+                                                         const uint2* __restrict__ ga, const float2* __restrict__ gb,
+                                                         const float2* __restrict__ gc, float2* __restrict__ grid) {
+    constexpr int h = (S - 1) / 2;
+    constexpr int kPasses = (S + RB - 1) / RB;
+    constexpr int W = S + 1;                    // even-aligned window, see k_grid_runs
+    constexpr int PPT = L / 2;                  // 16-byte pieces (two records) per thread and stream
+    constexpr int NP = kRunThreads * PPT;       // pieces per stream and CTA
+    static_assert(PPT >= 8 && (PPT & (PPT - 1)) == 0, "L must be a power of two >= 16");
+    extern __shared__ uint4 stage[];            // [3][NP]
+    const long long n = *n_kept;
+    const long long cta_first = (long long)blockIdx.x * (kRunThreads * L);
+    if (cta_first >= n) return;
+    const int tid = threadIdx.x;
+    {
+        const uint4* sa = (const uint4*)(ga + cta_first);
+        const uint4* sb = (const uint4*)(gb + cta_first);
+        const uint4* sc = (const uint4*)(gc + cta_first);
+#pragma unroll 4
+        for (int q = tid; q < NP; q += kRunThreads) {
+            const int phys = q ^ ((q / PPT) & 7);     // piece q belongs to thread q / PPT
+            cp_async16(stage + phys, sa + q);
+            cp_async16(stage + NP + phys, sb + q);
+            cp_async16(stage + 2 * NP + phys, sc + q);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    const long long first = cta_first + (long long)tid * L;
+    const int cnt = (n - first) >= L ? L : (int)(n - first);      // <= 0: nothing for this thread
+    if (cnt <= 0) return;
+    const size_t N = (size_t)g.N;
+    const float c2 = (float)(-g.tap_c * 1.4426950408889634);
+    const uint4* my = stage + tid * PPT;
+    const int sw = tid & 7;
+
+#pragma unroll
+    for (int pass = 0; pass < kPasses; ++pass) {
+        const int b0 = pass * RB;
+        float ar[RB][W], ai[RB][W];
+#pragma unroll
+        for (int r = 0; r < RB; ++r)
+#pragma unroll
+            for (int a = 0; a < W; ++a) ar[r][a] = ai[r][a] = 0.f;
+        uint32_t cij = 0xFFFFFFFFu, ck = 0;
+
+        auto flush = [&]() {
+            const int ci = (int)(cij & 0xFFFFu), cj = (int)(cij >> 16);
+            const int iw = (ci - h) & ~1;
+            float2* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)iw;
+            const bool edge = iw + W > (int)N;      // the zero column would fall past the row (i0 = N-1-h)
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                if (b0 + r < S) {
+#pragma unroll
+                    for (int a = 0; a < W; a += 2) {
+                        float2* dst = base + (size_t)r * N + a;
+                        if (a + 2 == W && edge) red_add_cell(dst, ar[r][a], ai[r][a]);
+                        else red_add_pair(dst, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
+                        ar[r][a] = ai[r][a] = ar[r][a + 1] = ai[r][a + 1] = 0.f;
+                    }
+                }
+            }
+        };
+
+        auto one = [&](uint32_t ij, uint32_t k, float dx, float dy, float vr, float vi) {
+            if (ij != cij || k != ck) {
+                if (cij != 0xFFFFFFFFu) flush();
+                cij = ij; ck = k;
+            }
+            float t[S], gx[W], gy[S];
+            taps_f32<S, true>(gy, dy, c2, tc);
+            taps_f32<S, false>(t, dx, c2, tc);
+            const bool o = (((int)(ij & 0xFFFFu) - h) & 1) != 0;     // footprint starts on an odd column
+#pragma unroll
+            for (int c = 0; c < W; ++c) {
+                const float lo = (c >= 1) ? t[c - 1] : 0.f, hi = (c < S) ? t[c] : 0.f;
+                const float v = o ? lo : hi;
+                gx[c] = (c & 1) ? -v : v;
+            }
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                if (b0 + r < S) {
+                    const float yr = gy[b0 + r] * vr, yi = gy[b0 + r] * vi;
+#pragma unroll
+                    for (int a = 0; a < W; ++a) {
+                        ar[r][a] = fmaf(gx[a], yr, ar[r][a]);
+                        ai[r][a] = fmaf(gx[a], yi, ai[r][a]);
+                    }
+                }
+            }
+        };
+
+#pragma unroll 1
+        for (int i = 0; i < cnt; i += 2) {
+            const int piece = (i >> 1) ^ sw;
+            const uint4 a = my[piece];
+            const uint4 b = my[NP + piece];
+            const uint4 c = my[2 * NP + piece];
+            one(a.x, a.y, __uint_as_float(b.x), __uint_as_float(b.y), __uint_as_float(c.x), __uint_as_float(c.y));
+            if (i + 1 < cnt)
+                one(a.z, a.w, __uint_as_float(b.z), __uint_as_float(b.w), __uint_as_float(c.z), __uint_as_float(c.w));
+        }
+        if (cij != 0xFFFFFFFFu) flush();
+    }
+}
+
+template <int S, int RB>
+int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
+    constexpr int L = kRunItems;
+    constexpr int smem = 3 * kRunThreads * (L / 2) * 16;
+    static bool attr_done = false;
+    if (!attr_done) {
+        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+            return RICK_ECUDA;
+        attr_done = true;
+    }
+    static_assert(kRunThreads * L <= RICK_GREC_PAD, "a CTA's records must lie inside the padded record arrays");
+    TapConst tc;
+    for (int t = 0; t < 8; ++t) {
+        tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
+        tc.Kf[t] = (float)tc.K[t];
+    }
+    const long long per_block = (long long)kRunThreads * L;
+    const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
+    k_grid_rec<S, RB, L><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
+                                                           (float2*)grid);
+    return RICK_OK;
+}
+
 template <typename real, int S, int RB>
 void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
     typedef typename CellOf<real>::type cell;
@@ -251,17 +398,19 @@ void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
 int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st) {
     if (p->M == 0) return RICK_OK;
     const bool f64 = (p->dtype == RICK_C128);
-    // <real, S, RB>: RB rows of the footprint are held in registers per pass (2*RB*S accumulators)
+    // <real, S, RB>: RB rows of the footprint are held in registers per pass
+    int rc = RICK_OK;
     switch (p->g.S) {
-        case 3:  f64 ? launch_runs<double, 3, 3>(p, grid, st)  : launch_runs<float, 3, 3>(p, grid, st); break;
-        case 5:  f64 ? launch_runs<double, 5, 5>(p, grid, st)  : launch_runs<float, 5, 5>(p, grid, st); break;
-        case 7:  f64 ? launch_runs<double, 7, 4>(p, grid, st)  : launch_runs<float, 7, 7>(p, grid, st); break;
-        case 9:  f64 ? launch_runs<double, 9, 3>(p, grid, st)  : launch_runs<float, 9, 5>(p, grid, st); break;
-        case 11: f64 ? launch_runs<double, 11, 2>(p, grid, st) : launch_runs<float, 11, 4>(p, grid, st); break;
-        case 13: f64 ? launch_runs<double, 13, 2>(p, grid, st) : launch_runs<float, 13, 3>(p, grid, st); break;
-        case 15: f64 ? launch_runs<double, 15, 2>(p, grid, st) : launch_runs<float, 15, 3>(p, grid, st); break;
+        case 3:  if (f64) launch_runs<double, 3, 3>(p, grid, st);  else rc = launch_rec<3, 3>(p, grid, st); break;
+        case 5:  if (f64) launch_runs<double, 5, 5>(p, grid, st);  else rc = launch_rec<5, 5>(p, grid, st); break;
+        case 7:  if (f64) launch_runs<double, 7, 4>(p, grid, st);  else rc = launch_rec<7, 7>(p, grid, st); break;
+        case 9:  if (f64) launch_runs<double, 9, 3>(p, grid, st);  else rc = launch_rec<9, 5>(p, grid, st); break;
+        case 11: if (f64) launch_runs<double, 11, 2>(p, grid, st); else rc = launch_rec<11, 4>(p, grid, st); break;
+        case 13: if (f64) launch_runs<double, 13, 2>(p, grid, st); else rc = launch_rec<13, 3>(p, grid, st); break;
+        case 15: if (f64) launch_runs<double, 15, 2>(p, grid, st); else rc = launch_rec<15, 3>(p, grid, st); break;
         default: return RICK_EINVAL;
     }
+    if (rc != RICK_OK) return rc;
     RICK_LAUNCH_CHECK();
     p->launches++;
     return RICK_OK;

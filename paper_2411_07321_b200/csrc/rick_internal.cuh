@@ -10,6 +10,7 @@
 
 #define RICK_TILE 32          // uv tile edge of the sort key (BASELINE.json north_star (2))
 #define RICK_MAX_PASSES 4
+#define RICK_GREC_PAD 4096    // gridder records are allocated in whole chunks of this many (one CTA's share)
 #define RICK_RADIX_BITS_MAX 9
 
 // Geometry constants handed to kernels by value.
@@ -48,6 +49,10 @@ struct rick_plan {
     const float *u_s, *v_s, *w_s, *weight_s;
     const void* vis_s;
     const long long* n_kept_dev;
+    // gridder records of the sorted kept visibilities, written by rick_bin's gather into its workspace:
+    //   a = (i0 | j0 << 16, k), b = (i0 - x, j0 - y) in fp32, c = +-weight * (re, im)
+    const uint2* grec_a;
+    const float2 *grec_b, *grec_c;
     // stage timing
     cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
     bool ev_valid[RICK_T_COUNT];
