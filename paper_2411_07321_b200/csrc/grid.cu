@@ -250,40 +250,41 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 template <int S, int RB, int L>
 __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                          const uint2* __restrict__ ga, const float2* __restrict__ gb,
-                                                         const float2* __restrict__ gc, float2* __restrict__ grid) {
+                                                         const float2* __restrict__ gc, float2* __restrict__ grid,
+                                                         int n_stage) {
     constexpr int h = (S - 1) / 2;
     constexpr int kPasses = (S + RB - 1) / RB;
     constexpr int W = S + 1;                    // even-aligned window, see k_grid_runs
-    constexpr int PPT = L / 2;                  // 16-byte pieces (two records) per thread and stream
-    constexpr int NP = kRunThreads * PPT;       // pieces per stream and CTA
+    constexpr int PPT = L / 2;                  // 16-byte pieces (two records) per thread, stream and stage
+    constexpr int NP = kRunThreads * PPT;       // pieces per stream and stage
     static_assert(PPT >= 8 && (PPT & (PPT - 1)) == 0, "L must be a power of two >= 16");
-    extern __shared__ uint4 stage[];            // [3][NP]
+    extern __shared__ uint4 stage[];            // [2 buffers][3 streams][NP]
     const long long n = *n_kept;
-    const long long cta_first = (long long)blockIdx.x * (kRunThreads * L);
+    const long long per_thread = (long long)L * n_stage;
+    const long long cta_first = (long long)blockIdx.x * (kRunThreads * per_thread);
     if (cta_first >= n) return;
     const int tid = threadIdx.x;
-    {
-        const uint4* sa = (const uint4*)(ga + cta_first);
-        const uint4* sb = (const uint4*)(gb + cta_first);
-        const uint4* sc = (const uint4*)(gc + cta_first);
-#pragma unroll 4
-        for (int q = tid; q < NP; q += kRunThreads) {
-            const int phys = q ^ ((q / PPT) & 7);     // piece q belongs to thread q / PPT
-            cp_async16(stage + phys, sa + q);
-            cp_async16(stage + NP + phys, sb + q);
-            cp_async16(stage + 2 * NP + phys, sc + q);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-    }
-    __syncthreads();
-    const long long first = cta_first + (long long)tid * L;
-    const int cnt = (n - first) >= L ? L : (int)(n - first);      // <= 0: nothing for this thread
-    if (cnt <= 0) return;
+    const long long first = cta_first + (long long)tid * per_thread;   // the thread's run of records
     const size_t N = (size_t)g.N;
     const float c2 = (float)(-g.tap_c * 1.4426950408889634);
-    const uint4* my = stage + tid * PPT;
     const int sw = tid & 7;
+
+    // stage st of every thread's range -> buffer st & 1 (16 lanes copy one thread's 16 * PPT bytes per stream)
+    auto issue = [&](int st) {
+        uint4* buf = stage + (st & 1) * (3 * NP);
+#pragma unroll 4
+        for (int q = tid; q < NP; q += kRunThreads) {
+            const int t = q / PPT, piece = q % PPT;
+            const long long rec = cta_first + (long long)t * per_thread + (long long)st * L + 2 * piece;
+            if (rec < n) {
+                const int phys = q ^ (t & 7);
+                cp_async16(buf + phys, (const uint4*)(ga + rec));
+                cp_async16(buf + NP + phys, (const uint4*)(gb + rec));
+                cp_async16(buf + 2 * NP + phys, (const uint4*)(gc + rec));
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
 
 #pragma unroll
     for (int pass = 0; pass < kPasses; ++pass) {
@@ -342,15 +343,28 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             }
         };
 
+        if (pass > 0) __syncthreads();          // every thread is done with both buffers
+        issue(0);
 #pragma unroll 1
-        for (int i = 0; i < cnt; i += 2) {
-            const int piece = (i >> 1) ^ sw;
-            const uint4 a = my[piece];
-            const uint4 b = my[NP + piece];
-            const uint4 c = my[2 * NP + piece];
-            one(a.x, a.y, __uint_as_float(b.x), __uint_as_float(b.y), __uint_as_float(c.x), __uint_as_float(c.y));
-            if (i + 1 < cnt)
-                one(a.z, a.w, __uint_as_float(b.z), __uint_as_float(b.w), __uint_as_float(c.z), __uint_as_float(c.w));
+        for (int st = 0; st < n_stage; ++st) {
+            if (st + 1 < n_stage) issue(st + 1);
+            else asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            __syncthreads();
+            const long long left = n - (first + (long long)st * L);
+            const int cnt = left >= L ? L : (left > 0 ? (int)left : 0);
+            const uint4* my = stage + (st & 1) * (3 * NP) + tid * PPT;
+#pragma unroll 1
+            for (int i = 0; i < cnt; i += 2) {
+                const int piece = (i >> 1) ^ sw;
+                const uint4 a = my[piece];
+                const uint4 b = my[NP + piece];
+                const uint4 c = my[2 * NP + piece];
+                one(a.x, a.y, __uint_as_float(b.x), __uint_as_float(b.y), __uint_as_float(c.x), __uint_as_float(c.y));
+                if (i + 1 < cnt)
+                    one(a.z, a.w, __uint_as_float(b.z), __uint_as_float(b.w), __uint_as_float(c.z), __uint_as_float(c.w));
+            }
+            __syncthreads();                    // buffer st & 1 is free for stage st + 2
         }
         if (cij != 0xFFFFFFFFu) flush();
     }
@@ -358,24 +372,28 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 
 template <int S, int RB>
 int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
-    constexpr int L = kRunItems;
-    constexpr int smem = 3 * kRunThreads * (L / 2) * 16;
+    constexpr int L = 16;                                   // records per thread and stage
+    constexpr int smem = 2 * 3 * kRunThreads * (L / 2) * 16;   // two buffers of three streams: 96 KB
     static bool attr_done = false;
     if (!attr_done) {
         if (cudaFuncSetAttribute(k_grid_rec<S, RB, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return RICK_ECUDA;
         attr_done = true;
     }
-    static_assert(kRunThreads * L <= RICK_GREC_PAD, "a CTA's records must lie inside the padded record arrays");
     TapConst tc;
     for (int t = 0; t < 8; ++t) {
         tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
         tc.Kf[t] = (float)tc.K[t];
     }
-    const long long per_block = (long long)kRunThreads * L;
+    // records per thread: long enough that end-of-range flushes are rare next to run ends (dense inputs
+    // put thousands of visibilities on one cell), short enough for >= ~12 CTAs per SM slot
+    const long long want = p->M / ((long long)kRunThreads * p->sm_count * 2 * 12);
+    int n_stage = (int)(want / L);
+    n_stage = n_stage < 2 ? 2 : (n_stage > 16 ? 16 : n_stage);
+    const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
     k_grid_rec<S, RB, L><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
-                                                           (float2*)grid);
+                                                           (float2*)grid, n_stage);
     return RICK_OK;
 }
 
