@@ -3,7 +3,7 @@
 // Run-accumulating gridder.  rick_bin leaves the kept visibilities sorted by (plane, tile, cell) [D4'],
 // so visibilities that share a nearest cell (i0, j0, k) -- and therefore the same S x S footprint --
 // are adjacent: 87 % of the "10M" workload sits in runs of >= 8.
-// Each thread walks kRunItems consecutive sorted visibilities and keeps the whole footprint
+// Each thread walks a range of consecutive sorted visibilities (32 .. 256) and keeps the whole footprint
 // (S*S complex accumulators, or a block of RB rows of it per pass) in registers:
 //
 //     acc[b][a] += gx[a] * (gy[b] * weight * V)          2 FMAs per cell and visibility
@@ -12,7 +12,7 @@
 // vector reductions in L2 (red.global.add.v4.f32, two cells each / red.global.add.f64).  Lanes of a warp hold
 // neighbouring cells, so those reductions fall into the same few sectors.  No shared memory, no
 // shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on sm_100a), and the number
-// of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to kRunItems).
+// of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to the range).
 //
 // The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) costs nothing: (-1)^(a+b) is folded
 // into the taps as compile-time negations and (-1)^(i0+j0) into the sign of the weight.
@@ -21,10 +21,6 @@
 namespace {
 
 constexpr int kRunThreads = 128;
-#ifndef RICK_RUN_ITEMS
-#define RICK_RUN_ITEMS 32
-#endif
-constexpr int kRunItems = RICK_RUN_ITEMS;   // consecutive sorted visibilities per thread (a multiple of 8)
 
 struct TapConst {
     double K[8];   // K[t] = exp(-t^2 / (2 sigma^2)), t = 0 .. h
@@ -94,10 +90,6 @@ __device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, co
     }
 }
 
-__device__ __forceinline__ void prefetch_l1(const void* p) {
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-}
-
 template <typename real> struct CellOf;
 template <> struct CellOf<float> { typedef float2 type; };
 template <> struct CellOf<double> { typedef double2 type; };
@@ -112,12 +104,12 @@ __device__ __forceinline__ float4 load4(const float* __restrict__ a, long long p
     return r;
 }
 
-template <typename real, int S, int RB, int L>
+template <typename real, int S, int RB>
 __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                           const float* __restrict__ u_s, const float* __restrict__ v_s,
                                                           const float* __restrict__ w_s, const float2* __restrict__ vis_s,
                                                           const float* __restrict__ wt_s,
-                                                          typename CellOf<real>::type* __restrict__ grid) {
+                                                          typename CellOf<real>::type* __restrict__ grid, int L) {
     typedef typename CellOf<real>::type cell;
     constexpr int h = (S - 1) / 2;
     constexpr int kPasses = (S + RB - 1) / RB;
@@ -126,19 +118,9 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
     constexpr bool kWin = (sizeof(real) == 4);
     constexpr int W = kWin ? S + 1 : S;
     const long long n = *n_kept;
-    const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * L;
+    const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * L;   // L: a multiple of 4
     if (first >= n) return;
     const size_t N = (size_t)g.N;
-    // pull the thread's 32-B sectors into L1 before the first use (the loads below then hit)
-#pragma unroll
-    for (int q = 0; q < L / 8; ++q) {
-        prefetch_l1(u_s + first + 8 * q);
-        prefetch_l1(v_s + first + 8 * q);
-        prefetch_l1(w_s + first + 8 * q);
-        prefetch_l1(wt_s + first + 8 * q);
-        prefetch_l1(vis_s + first + 8 * q);
-        prefetch_l1(vis_s + first + 8 * q + 4);
-    }
 
 #pragma unroll
     for (int pass = 0; pass < kPasses; ++pass) {
@@ -405,10 +387,14 @@ void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
         tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
         tc.Kf[t] = (float)tc.K[t];
     }
-    const long long per_block = (long long)kRunThreads * kRunItems;
+    // consecutive sorted visibilities per thread: as for the record gridder, long ranges on dense inputs
+    // (fewer end-of-range reductions onto the same hot cells), >= ~12 CTAs per SM slot
+    long long L = p->M / ((long long)kRunThreads * p->sm_count * 2 * 12) / 4 * 4;
+    L = L < 32 ? 32 : (L > 256 ? 256 : L);
+    const long long per_block = (long long)kRunThreads * L;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
-    k_grid_runs<real, S, RB, kRunItems><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
-                                                              (const float2*)p->vis_s, p->weight_s, (cell*)grid);
+    k_grid_runs<real, S, RB><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
+                                                              (const float2*)p->vis_s, p->weight_s, (cell*)grid, (int)L);
 }
 
 }  // namespace
