@@ -175,6 +175,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fusion", action="store_true", help="2-D cuFFT + separate w-correction kernel")
     ap.add_argument("--e2e-steps", type=int, default=5)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -203,7 +204,7 @@ def main():
     vis = W.generate(cfg, device=dev)
     pa = W.plan_args(cfg, vis)
     M = vis.M
-    im = B.Imager(dtype=cfg.dtype, M_max=M, **pa)
+    im = B.Imager(dtype=cfg.dtype, M_max=M, fused=not args.no_fusion, **pa)
     cell = 16 if cfg.dtype == "c128" else 8
     mesh_bytes = cfg.Nw * cfg.N * cfg.N * cell
 
@@ -255,8 +256,8 @@ def main():
         "gather": (4 + 32 + 24) * n_kept,            # index + record in, sorted SoA out
         "zero": mesh_bytes,
         "grid": 24 * n_kept,
-        "fft": 4 * mesh_bytes,
-        "wcorrect": mesh_bytes + cfg.N * cfg.N * 8,
+        "fft": (2 if im.fused else 4) * mesh_bytes,      # fused: row transforms only (one read + write)
+        "wcorrect": mesh_bytes + cfg.N * cfg.N * 8,      # fused: column transforms + screen + sum, one read
     }
     stages = {}
     for k, b in alg.items():
@@ -270,7 +271,8 @@ def main():
                            "vis_per_s": n_kept / (zg * 1e-3)}
     # the dominant kernel = the library kernel with the largest total time in a step; its roofline numbers
     # are per launch (sort: n_pass launches of k_onesweep, the average pass)
-    kernels = {"grid": ("k_grid_runs", 1), "wcorrect": ("k_wcorrect", 1), "keygen": ("k_keygen", 1),
+    kernels = {"grid": ("k_grid_rec" if cfg.dtype == "c64" else "k_grid_runs", 1),
+               "wcorrect": ("k_colfft_wcorrect" if im.fused else "k_wcorrect", 1), "keygen": ("k_keygen", 1),
                "sort": ("k_onesweep", n_pass), "gather": ("k_gather", 1)}
     dom = max(kernels, key=lambda k: stage_ms[k])
     kname, n_launch = kernels[dom]
@@ -314,7 +316,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
         "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
-                   "support": cfg.support, "sigma": cfg.sigma, "mesh": cfg.dtype,
+                   "support": cfg.support, "sigma": cfg.sigma, "mesh": cfg.dtype, "fused_column_transform": bool(im.fused),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs (240 MB) and mesh (1.07 GB) exceed the 126 MB L2; no explicit flush"
                    if args.config == "10M" else "inputs and mesh exceed L2; no explicit flush"},

@@ -77,6 +77,13 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
 /* Select the mesh dtype and (re)build the cuFFT plan for it.  Host-synchronous. */
 int rick_plan_set_dtype(rick_plan* plan, int dtype);
 
+/* Fused column transform (optional; RICK_C64 and N in {256, 512, 1024, 2048} only, RICK_EINVAL otherwise;
+ * call after rick_plan_set_dtype, which switches it off).  With fusion on, rick_fft_planes runs only the
+ * row transforms of D7 (the mesh then holds row-transformed planes), and rick_wcorrect_accumulate
+ * performs the column transforms itself, fused with the phase screen, the plane sum and the taper
+ * division, in one read of the mesh [D7, D8].  The image is the same within fp32 round-off. */
+int rick_plan_set_fusion(rick_plan* plan, int on);
+
 /* Sizes of the two caller-provided scratch buffers: `bin_bytes` for rick_bin with up to M
  * visibilities, `fft_bytes` for rick_fft_planes (0 if cuFFT needs none).  Either pointer may be NULL. */
 int rick_plan_workspace_bytes(const rick_plan* plan, long long M, size_t* bin_bytes, size_t* fft_bytes);

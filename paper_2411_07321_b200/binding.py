@@ -21,7 +21,7 @@ _lib = None
 
 EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
-    "rick_plan_sort_layout",
+    "rick_plan_sort_layout", "rick_plan_set_fusion",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
@@ -61,6 +61,7 @@ def lib():
         L.rick_plan_set_dtype.argtypes = [vp, i]
         L.rick_plan_workspace_bytes.argtypes = [vp, ll, C.POINTER(sz), C.POINTER(sz)]
         L.rick_plan_destroy.argtypes = [vp]
+        L.rick_plan_set_fusion.argtypes = [vp, i]
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
@@ -124,6 +125,15 @@ def rick_plan_sort_layout(plan: int):
     a, b, c = C.c_int(), C.c_int(), C.c_int()
     _check(lib().rick_plan_sort_layout(plan, C.byref(a), C.byref(b), C.byref(c)), "rick_plan_sort_layout")
     return int(a.value), int(b.value), int(c.value)
+
+
+def rick_plan_set_fusion(plan: int, on: bool) -> bool:
+    """Switch the fused column-transform + w-correction path on/off; False when the plan does not support it."""
+    rc = lib().rick_plan_set_fusion(plan, 1 if on else 0)
+    if rc == -1 and on:      # RICK_EINVAL: dtype / N not supported by the fused kernel
+        return False
+    _check(rc, "rick_plan_set_fusion")
+    return bool(on)
 
 
 def rick_plan_destroy(plan: int) -> None:
@@ -193,7 +203,7 @@ class Imager:
     points in path order.  Nothing is computed in Python."""
 
     def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
-                 dtype: str = "c64", M_max: int = 0, device="cuda"):
+                 dtype: str = "c64", M_max: int = 0, device="cuda", fused: bool = False):
         if not torch.cuda.is_available():
             raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -203,6 +213,7 @@ class Imager:
         with torch.cuda.device(self.device):
             self.plan = rick_plan_create(N, Nw, support, sigma, w_min, w_max, dl)
             rick_plan_set_dtype(self.plan, self.dtype)
+            self.fused = rick_plan_set_fusion(self.plan, True) if fused else False
         self.M_max = 0
         self.grid = torch.empty((Nw, N, N), dtype=self.cdtype, device=self.device)
         self.image = torch.empty((N, N), dtype=torch.float64, device=self.device)

@@ -1,0 +1,285 @@
+// colfft.cu -- fused column transform + w-correction (RICK_C64, N = 256 .. 2048, opt-in through
+// rick_plan_set_fusion): the second half of D7 and all of D8 in ONE read of the mesh.
+//
+// With fusion on, rick_fft_planes only runs the contiguous row transforms (batched 1-D cuFFT, which
+// streams at the copy rate); the strided column pass -- the slow half of a 2-D cuFFT (profiles/) -- is
+// done here.  A CTA owns kC = 4 adjacent image columns.  For every plane it pulls the N x 4 column block
+// (32-byte rows, full sectors) into shared memory with cp.async (double-buffered against the next
+// plane), runs four in-place length-N inverse DFTs (decimation in frequency, radix 16 x 16 x {1,2,4,8},
+// butterflies in registers, digit-reversed output left in place), multiplies each output by the phase
+// screen exp(+2 pi i w_k nm1(q,p)) (Eq. 2) and adds the real part to fp64 accumulators that stay
+// in registers for all planes.  At the end: (-1)^(p+q), the taper division, one write of the image.
+// The transformed planes are never written back: the column pass of a 2-D FFT (read + write of the
+// mesh) and the K5 sweep (another read) collapse into one read.
+//
+// Phase: w_k * nm1 reduced to [-1/2, 1/2] turns in fp64 (nm1 per pixel kept in shared memory), then the
+// hardware sine / cosine in fp32 on the reduced argument (abs error < 5e-7, the precision of the fp32
+// planes themselves); the product in fp32, the plane sum in fp64.
+#include "rick_internal.cuh"
+
+namespace {
+
+constexpr int kC = 4;            // columns per CTA
+constexpr int kT = 512;          // threads per CTA
+constexpr int kPadShift = 5;     // 4 float2 of padding after every 32 float2 (bank-conflict-free passes)
+
+__device__ __forceinline__ int padded(int idx) { return idx + ((idx >> kPadShift) << 2); }
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// 4-point inverse DFT (omega_4 = +i), in place
+__device__ __forceinline__ void dft4(float2& a, float2& b, float2& c, float2& d) {
+    const float2 s0 = make_float2(a.x + c.x, a.y + c.y), d0 = make_float2(a.x - c.x, a.y - c.y);
+    const float2 s1 = make_float2(b.x + d.x, b.y + d.y), d1 = make_float2(b.x - d.x, b.y - d.y);
+    a = make_float2(s0.x + s1.x, s0.y + s1.y);
+    c = make_float2(s0.x - s1.x, s0.y - s1.y);
+    b = make_float2(d0.x - d1.y, d0.y + d1.x);      // d0 + i d1
+    d = make_float2(d0.x + d1.y, d0.y - d1.x);      // d0 - i d1
+}
+
+// R-point inverse DFT, y_u = sum_t x_t exp(+2 pi i u t / R), natural order in and out
+template <int R> __device__ __forceinline__ void dft(float2* v);
+template <> __device__ __forceinline__ void dft<1>(float2*) {}
+template <> __device__ __forceinline__ void dft<2>(float2* v) {
+    const float2 a = v[0], b = v[1];
+    v[0] = make_float2(a.x + b.x, a.y + b.y);
+    v[1] = make_float2(a.x - b.x, a.y - b.y);
+}
+template <> __device__ __forceinline__ void dft<4>(float2* v) { dft4(v[0], v[1], v[2], v[3]); }
+template <> __device__ __forceinline__ void dft<8>(float2* v) {
+    float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
+    dft4(e0, e1, e2, e3);
+    dft4(o0, o1, o2, o3);
+    const float r = 0.70710678118654752f;
+    const float2 t1 = make_float2(r * (o1.x - o1.y), r * (o1.x + o1.y));     // o1 * exp(+i pi/4)
+    const float2 t2 = make_float2(-o2.y, o2.x);                               // o2 * i
+    const float2 t3 = make_float2(-r * (o3.x + o3.y), r * (o3.x - o3.y));    // o3 * exp(+3 i pi/4)
+    v[0] = make_float2(e0.x + o0.x, e0.y + o0.y); v[4] = make_float2(e0.x - o0.x, e0.y - o0.y);
+    v[1] = make_float2(e1.x + t1.x, e1.y + t1.y); v[5] = make_float2(e1.x - t1.x, e1.y - t1.y);
+    v[2] = make_float2(e2.x + t2.x, e2.y + t2.y); v[6] = make_float2(e2.x - t2.x, e2.y - t2.y);
+    v[3] = make_float2(e3.x + t3.x, e3.y + t3.y); v[7] = make_float2(e3.x - t3.x, e3.y - t3.y);
+}
+// 16 = 4 x 4: t = 4a + b, u = c + 4d:  w16^(ut) = w4^(ac) w16^(bc) w4^(bd)
+template <> __device__ __forceinline__ void dft<16>(float2* v) {
+#pragma unroll
+    for (int b = 0; b < 4; ++b) dft4(v[b], v[4 + b], v[8 + b], v[12 + b]);   // over a: result c at v[4c + b]
+    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, r = 0.70710678118654752f;
+    const float2 w1 = make_float2(c1, s1), w2 = make_float2(r, r), w3 = make_float2(s1, c1);
+    const float2 w6 = make_float2(-r, r), w9 = make_float2(-c1, -s1);
+    // z(b,c) at v[4c + b] *= w16^(bc)
+    v[4 + 1] = cmul(v[4 + 1], w1); v[4 + 2] = cmul(v[4 + 2], w2); v[4 + 3] = cmul(v[4 + 3], w3);
+    v[8 + 1] = cmul(v[8 + 1], w2); v[8 + 2] = make_float2(-v[8 + 2].y, v[8 + 2].x); v[8 + 3] = cmul(v[8 + 3], w6);
+    v[12 + 1] = cmul(v[12 + 1], w3); v[12 + 2] = cmul(v[12 + 2], w6); v[12 + 3] = cmul(v[12 + 3], w9);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) dft4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);   // over b: d at v[4c + d]
+    // y(c + 4d) sits at v[4c + d]: transpose the 4 x 4 so that y_u is at v[u]
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int d = c + 1; d < 4; ++d) {
+            const float2 t = v[4 * c + d];
+            v[4 * c + d] = v[4 * d + c];
+            v[4 * d + c] = t;
+        }
+}
+
+// One in-place decimation-in-frequency pass of radix R over sub-transforms of length n = 2^LOG2n of the
+// N = 2^LOG2N point columns:  for every sub-block B, offset m < n/R, column c:
+//   x[B n + m + t n/R], t < R  ->  R-point DFT  ->  y_u * W_n^(m u) stored at the same slots (u for t).
+// tw[j] = exp(+2 pi i j / N).  Everything but m is a compile-time constant: the R slots of a butterfly
+// are the padded base plus constant offsets.
+template <int LOG2N, int R, int LOG2n>
+__device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid) {
+    constexpr int N = 1 << LOG2N, n = 1 << LOG2n;
+    constexpr int q = n / R;                     // stride between the R inputs (rows)
+    constexpr int stride = q * kC;               // ... in float2 slots
+    constexpr int per_block = stride;            // butterflies per sub-block = q * kC
+    constexpr int total = N * kC / R;            // butterflies per pass
+    constexpr int tw_step = N / n;
+    constexpr bool kConstOff = (stride % 32) == 0 || (R * stride <= 32);   // padding is affine over the butterfly
+#pragma unroll
+    for (int w0 = 0; w0 < total; w0 += kT) {
+        const int w = w0 + tid;
+        if (total % kT != 0 && w >= total) break;
+        const int B = w / per_block, rem = w % per_block;     // powers of two: shifts
+        const int base = B * (n * kC) + rem;                  // ((B n + m) kC + c), rem = m kC + c
+        const int pb = padded(base);
+        float2 v[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t)
+            v[t] = kConstOff ? buf[pb + t * (stride + ((stride >> kPadShift) << 2))] : buf[padded(base + t * stride)];
+        dft<R>(v);
+        if (q > 1) {
+            const int ts = (rem / kC) * tw_step;              // m * N / n
+            int idx = 0;
+#pragma unroll
+            for (int u = 1; u < R; ++u) {
+                idx = (idx + ts) & (N - 1);
+                v[u] = cmul(v[u], tw[idx]);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < R; ++u) {
+            if (kConstOff) buf[pb + u * (stride + ((stride >> kPadShift) << 2))] = v[u];
+            else buf[padded(base + u * stride)] = v[u];
+        }
+    }
+}
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+
+// digit-reversed slot -> frequency: slot = u1 N/16 + u2 N/256 + u3  ->  q = u1 + 16 u2 + 256 u3
+__device__ __forceinline__ int slot_to_freq(int slot, int N) {
+    const int u1 = slot / (N >> 4), r1 = slot - u1 * (N >> 4);
+    const int u2 = r1 / (N >> 8), u3 = r1 - u2 * (N >> 8);
+    return u1 + (u2 << 4) + (u3 << 8);
+}
+
+template <int LOG2N>
+__global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const float2* __restrict__ planes,
+                                                           const float2* __restrict__ tw_g,
+                                                           const double* __restrict__ inv_t,
+                                                           double* __restrict__ image, int accumulate) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int N = 1 << LOG2N;
+    constexpr int R3 = N >> 8;                        // radices 16 x 16 x R3
+    constexpr int n_slots = N * kC;                   // complex values of one column block
+    constexpr int buf_elems = n_slots + ((n_slots >> kPadShift) << 2);   // float2 per buffer
+    float2* buf0 = reinterpret_cast<float2*>(smem_raw);
+    float2* buf1 = buf0 + buf_elems;
+    float2* tw = buf1 + buf_elems;                    // [N]
+    double* nm1_s = reinterpret_cast<double*>(tw + N);   // [n_slots], indexed like the data (unpadded)
+    const int tid = threadIdx.x;
+    const int p0 = blockIdx.x * kC;
+    constexpr int per_thread = n_slots / kT;          // outputs owned by a thread: 2 .. 16
+
+    auto issue = [&](int k, float2* buf) {
+        const float2* src = planes + (size_t)k * N * N + p0;
+        // row j: kC float2 = 32 B = two 16-byte pieces
+        for (int q = tid; q < N * 2; q += kT) {
+            const int j = q >> 1, half = q & 1;
+            cp_async16(buf + padded(j * kC + half * 2), src + (size_t)j * N + half * 2);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    issue(0, buf0);
+    for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
+    for (int e = 0; e < per_thread; ++e) {
+        const int idx = e * kT + tid;
+        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
+        const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
+        const double r2 = l * l + m * m;
+        nm1_s[idx] = -r2 / (1.0 + sqrt(1.0 - r2));
+    }
+    double acc[16];                                   // per_thread <= 16 (N <= 2048)
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e] = 0.0;
+
+    for (int k = 0; k < g.Nw; ++k) {
+        float2* buf = (k & 1) ? buf1 : buf0;
+        if (k + 1 < g.Nw) issue(k + 1, (k & 1) ? buf0 : buf1);
+        else asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncthreads();
+        dif_pass<LOG2N, 16, LOG2N>(buf, tw, tid);
+        __syncthreads();
+        dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid);
+        __syncthreads();
+        if (R3 > 1) {
+            dif_pass<LOG2N, R3, LOG2N - 8>(buf, tw, tid);
+            __syncthreads();
+        }
+        const double wk = g.w_min + ((double)k + 0.5) * g.dw;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            if (e < per_thread) {
+                const int idx = e * kT + tid;
+                const float2 v = buf[padded(idx)];
+                double t = wk * nm1_s[idx];
+                t -= rint(t);                                  // [-1/2, 1/2] turns
+                float sn, cs;
+                __sincosf(6.283185307179586f * (float)t, &sn, &cs);   // MUFU on [-pi, pi]: abs error < 5e-7
+                acc[e] += (double)(cs * v.x - sn * v.y);
+            }
+        }
+        __syncthreads();                              // buf is free for plane k + 2
+    }
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        if (e < per_thread) {
+            const int idx = e * kT + tid;
+            const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
+            const double sg = ((p + q) & 1) ? -1.0 : 1.0;
+            double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
+            const size_t o = (size_t)q * N + p;
+            if (accumulate) out += image[o];
+            image[o] = out;
+        }
+    }
+}
+
+size_t colfft_smem_bytes(int N) {
+    const int n_slots = N * kC;
+    const size_t buf = (size_t)(n_slots + ((n_slots >> kPadShift) << 2)) * sizeof(float2);
+    return 2 * buf + (size_t)N * sizeof(float2) + (size_t)n_slots * sizeof(double);
+}
+
+}  // namespace
+
+bool rick_colfft_supported(const rick_plan* p) {
+    const int N = p->g.N;
+    return p->dtype == RICK_C64 && (N == 256 || N == 512 || N == 1024 || N == 2048);
+}
+
+int rick_colfft_init(rick_plan* p) {
+    // twiddles exp(+2 pi i j / N), fp64 values rounded once, on the device
+    const int N = p->g.N;
+    float2* h = (float2*)malloc(sizeof(float2) * (size_t)N);
+    if (!h) return RICK_ENOMEM;
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int j = 0; j < N; ++j) h[j] = make_float2((float)cos(two_pi * j / N), (float)sin(two_pi * j / N));
+    if (p->colfft_tw) { cudaFree(p->colfft_tw); p->colfft_tw = nullptr; }
+    cudaError_t e = cudaMalloc((void**)&p->colfft_tw, sizeof(float2) * (size_t)N);
+    if (e == cudaSuccess) e = cudaMemcpy(p->colfft_tw, h, sizeof(float2) * (size_t)N, cudaMemcpyHostToDevice);
+    free(h);
+    if (e != cudaSuccess) return RICK_ECUDA;
+    const int smem = (int)colfft_smem_bytes(N);
+    const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    cudaError_t ea = cudaSuccess;
+    switch (N) {
+        case 256: ea = cudaFuncSetAttribute(k_colfft_wcorrect<8>, a, smem); break;
+        case 512: ea = cudaFuncSetAttribute(k_colfft_wcorrect<9>, a, smem); break;
+        case 1024: ea = cudaFuncSetAttribute(k_colfft_wcorrect<10>, a, smem); break;
+        case 2048: ea = cudaFuncSetAttribute(k_colfft_wcorrect<11>, a, smem); break;
+        default: return RICK_EINVAL;
+    }
+    if (ea != cudaSuccess) return RICK_ECUDA;
+    return RICK_OK;
+}
+
+int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st) {
+    const RickGeom& g = p->g;
+    const int N = g.N;
+    const unsigned blocks = (unsigned)(N / kC);
+    const size_t smem = colfft_smem_bytes(N);
+    const float2* planes = (const float2*)grid;
+    const float2* tw = (const float2*)p->colfft_tw;
+    const int acc = zero_first ? 0 : 1;
+    switch (N) {
+        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
+        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
+        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
+        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
+        default: return RICK_EINVAL;
+    }
+    RICK_LAUNCH_CHECK();
+    p->launches++;
+    return RICK_OK;
+}

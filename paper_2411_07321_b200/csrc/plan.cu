@@ -38,6 +38,30 @@ void destroy_fft(rick_plan* p) {
         cufftDestroy(p->fft);
         p->fft_ready = false;
     }
+    if (p->fft_rows_ready) {
+        cufftDestroy(p->fft_rows);
+        p->fft_rows_ready = false;
+    }
+    p->fft_rows_work_bytes = 0;
+    p->fused = false;
+}
+
+// batched 1-D inverse transforms of all Nw * N rows, in place (the row half of D7)
+int build_fft_rows(rick_plan* p) {
+    const long long N = p->g.N;
+    cufftHandle h;
+    if (cufftCreate(&h) != CUFFT_SUCCESS) return RICK_ECUFFT;
+    if (cufftSetAutoAllocation(h, 0) != CUFFT_SUCCESS) { cufftDestroy(h); return RICK_ECUFFT; }
+    long long n[1] = {N};
+    size_t work = 0;
+    if (cufftMakePlanMany64(h, 1, n, NULL, 1, N, NULL, 1, N, CUFFT_C2C, N * p->g.Nw, &work) != CUFFT_SUCCESS) {
+        cufftDestroy(h);
+        return RICK_ECUFFT;
+    }
+    p->fft_rows = h;
+    p->fft_rows_ready = true;
+    p->fft_rows_work_bytes = work;
+    return RICK_OK;
 }
 
 // Largest batch (a divisor of Nw) whose cuFFT work area stays within `limit` bytes.
@@ -170,12 +194,26 @@ int rick_plan_set_dtype(rick_plan* p, int dtype) {
     return build_fft(p);
 }
 
+int rick_plan_set_fusion(rick_plan* p, int on) {
+    if (!p) return RICK_EINVAL;
+    if (!on) { p->fused = false; return RICK_OK; }
+    if (!p->dtype_set) return RICK_ESTATE;
+    if (!rick_colfft_supported(p)) return RICK_EINVAL;
+    if (!p->fft_rows_ready) {
+        int rc = build_fft_rows(p);
+        if (rc != RICK_OK) return rc;
+        if ((rc = rick_colfft_init(p)) != RICK_OK) return rc;
+    }
+    p->fused = true;
+    return RICK_OK;
+}
+
 int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes, size_t* fft_bytes) {
     if (!p || M < 0 || M >= 4294967295ll) return RICK_EINVAL;
     if (bin_bytes) *bin_bytes = rick_bin_workspace_bytes(p, M);
     if (fft_bytes) {
         if (!p->fft_ready) return RICK_ESTATE;
-        *fft_bytes = p->fft_work_bytes;
+        *fft_bytes = p->fft_work_bytes > p->fft_rows_work_bytes ? p->fft_work_bytes : p->fft_rows_work_bytes;
     }
     return RICK_OK;
 }
@@ -192,6 +230,7 @@ int rick_plan_destroy(rick_plan* p) {
     if (!p) return RICK_EINVAL;
     destroy_fft(p);
     if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
+    if (p->colfft_tw) cudaFree(p->colfft_tw);
     for (int i = 0; i < RICK_T_COUNT; ++i) {
         if (p->ev_start[i]) cudaEventDestroy(p->ev_start[i]);
         if (p->ev_stop[i]) cudaEventDestroy(p->ev_stop[i]);
@@ -232,6 +271,15 @@ int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_by
     if (!p->fft_ready) return RICK_ESTATE;
     if (p->fft_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_work_bytes)) return RICK_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
+    if (p->fused) {   // rows only; rick_wcorrect_accumulate finishes the transform (colfft.cu)
+        if (p->fft_rows_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_rows_work_bytes)) return RICK_ENOMEM;
+        if (cufftSetStream(p->fft_rows, st) != CUFFT_SUCCESS) return RICK_ECUFFT;
+        if (p->fft_rows_work_bytes > 0 && cufftSetWorkArea(p->fft_rows, fft_work) != CUFFT_SUCCESS) return RICK_ECUFFT;
+        StageTimer tm(p, RICK_T_FFT, st);
+        if (cufftExecC2C(p->fft_rows, (cufftComplex*)grid, (cufftComplex*)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
+            return RICK_ECUFFT;
+        return RICK_OK;
+    }
     if (cufftSetStream(p->fft, st) != CUFFT_SUCCESS) return RICK_ECUFFT;
     if (p->fft_work_bytes > 0 && cufftSetWorkArea(p->fft, fft_work) != CUFFT_SUCCESS) return RICK_ECUFFT;
     StageTimer tm(p, RICK_T_FFT, st);
@@ -254,6 +302,7 @@ int rick_wcorrect_accumulate(rick_plan* p, const void* grid, double* image, int 
     if (!p || !grid || !image) return RICK_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     StageTimer tm(p, RICK_T_WCORRECT, st);
+    if (p->fused) return rick_colfft_wcorrect_impl(p, grid, image, zero_first, st);
     return rick_wcorrect_impl(p, grid, image, zero_first, st);
 }
 

@@ -38,6 +38,12 @@ struct rick_plan {
     int digit_bits[RICK_MAX_PASSES], digit_shift[RICK_MAX_PASSES];
     // taper: inv_t[p] = 1 / t[p], device double[N]
     double* inv_taper_dev;
+    // fused column transform + w-correction (colfft.cu), opt-in
+    bool fused;              // rick_plan_set_fusion: rick_fft_planes does rows only, K6 finishes
+    cufftHandle fft_rows;    // batched 1-D row transforms
+    bool fft_rows_ready;
+    size_t fft_rows_work_bytes;
+    void* colfft_tw;         // device float2[N]: exp(+2 pi i j / N)
     // cuFFT
     cufftHandle fft;
     bool fft_ready;
@@ -129,3 +135,6 @@ size_t rick_bin_workspace_bytes(const rick_plan* p, long long M);
 int rick_bin_init();   // one-time kernel attributes (dynamic shared memory opt-in)
 int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st);
 int rick_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
+bool rick_colfft_supported(const rick_plan* p);
+int rick_colfft_init(rick_plan* p);
+int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);

@@ -248,3 +248,36 @@ def test_chunked_accumulation_and_host_entry():
     tm = im.timings()
     assert all(tm[k] > 0 for k in ("bin", "zero", "grid", "fft", "wcorrect", "image"))
     im.close()
+
+
+@pytest.mark.parametrize("name,M,plan", [
+    ("tiny", 100_000, dict(N=256, Nw=8)),                 # radix 16 x 16
+    ("10M", 300_000, dict(N=512, Nw=8)),                  # 16 x 16 x 2
+    ("100M", 300_000, dict(N=1024, Nw=16)),               # 16 x 16 x 4, wide field: the w term matters
+    ("10M", 1_000_003, dict(N=2048, Nw=32)),              # 16 x 16 x 8, the bench plan
+])
+def test_fused_column_transform(name, M, plan):
+    """rick_plan_set_fusion: row cuFFT + fused column transform / w-correction equals the oracle image
+    (same gates) and the unfused path; accumulate mode (zero_first = 0) adds."""
+    cfg, vis, pa = make(name, M, dtype="c64", **plan)
+    N = pa["N"]
+    im = B.Imager(dtype="c64", M_max=M, fused=True, **pa)
+    assert im.fused
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    ref = O.image(O.Plan(**pa), *vis.numpy())
+    a, b, full = gates(img, ref, N, cfg.support, cfg.sigma)
+    print(f"fused {name} N={N}: gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
+    assert a <= TOL["c64"] and b <= TOL["c64"]
+    im.grid_(True)
+    im.fft()
+    im.wcorrect(False)                                     # accumulate onto the image: twice the image
+    torch.cuda.synchronize()
+    twice = im.image.cpu().numpy()
+    t = O.taper(N, cfg.support, cfg.sigma)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    assert (np.abs(twice - 2 * img) * tw).max() <= 2e-6 * np.abs(img * tw).max()
+    im.close()
+    # a c128 plan or an unsupported size refuses fusion and stays on the two-kernel path
+    im2 = B.Imager(dtype="c128", M_max=16, fused=True, **pa)
+    assert not im2.fused
+    im2.close()
