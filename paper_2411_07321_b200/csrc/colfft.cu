@@ -112,13 +112,20 @@ __device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid)
             v[t] = kConstOff ? buf[pb + t * (stride + ((stride >> kPadShift) << 2))] : buf[padded(base + t * stride)];
         dft<R>(v);
         if (q > 1) {
+            // W_n^(m u), u < R: the powers of two come from the table, the rest are products of at
+            // most three of them (shared-memory bandwidth, not arithmetic, bounds this kernel)
             const int ts = (rem / kC) * tw_step;              // m * N / n
-            int idx = 0;
+            float2 wp[R];
 #pragma unroll
-            for (int u = 1; u < R; ++u) {
-                idx = (idx + ts) & (N - 1);
-                v[u] = cmul(v[u], tw[idx]);
-            }
+            for (int u = 1; u < R; u <<= 1) wp[u] = tw[(ts * u) & (N - 1)];
+#pragma unroll
+            for (int u = 3; u < R; ++u)
+                if (u & (u - 1)) {                            // not a power of two: lowest set bit times the rest
+                    const int lo = u & -u;
+                    wp[u] = cmul(wp[u - lo], wp[lo]);
+                }
+#pragma unroll
+            for (int u = 1; u < R; ++u) v[u] = cmul(v[u], wp[u]);
         }
 #pragma unroll
         for (int u = 0; u < R; ++u) {
@@ -169,7 +176,12 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    issue(0, buf0);
+    // planes of this CTA: gridDim.y splits the plane range (two halves fill the last wave of CTAs)
+    const int k_per = (g.Nw + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int k_lo = (int)blockIdx.y * k_per;
+    const int k_hi = (k_lo + k_per < g.Nw) ? k_lo + k_per : g.Nw;
+    if (k_lo >= k_hi) return;
+    issue(k_lo, buf0);
     for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
     for (int e = 0; e < per_thread; ++e) {
         const int idx = e * kT + tid;
@@ -182,9 +194,10 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 #pragma unroll
     for (int e = 0; e < 16; ++e) acc[e] = 0.0;
 
-    for (int k = 0; k < g.Nw; ++k) {
-        float2* buf = (k & 1) ? buf1 : buf0;
-        if (k + 1 < g.Nw) issue(k + 1, (k & 1) ? buf0 : buf1);
+    for (int k = k_lo; k < k_hi; ++k) {
+        const int par = (k - k_lo) & 1;
+        float2* buf = par ? buf1 : buf0;
+        if (k + 1 < k_hi) issue(k + 1, par ? buf0 : buf1);
         else asm volatile("cp.async.commit_group;" ::: "memory");
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncthreads();
@@ -219,8 +232,12 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
             const double sg = ((p + q) & 1) ? -1.0 : 1.0;
             double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
             const size_t o = (size_t)q * N + p;
-            if (accumulate) out += image[o];
-            image[o] = out;
+            if (gridDim.y > 1) {
+                atomicAdd(image + o, out);       // two addends onto a zeroed or given image: order-independent
+            } else {
+                if (accumulate) out += image[o];
+                image[o] = out;
+            }
         }
     }
 }
@@ -267,7 +284,12 @@ int rick_colfft_init(rick_plan* p) {
 int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st) {
     const RickGeom& g = p->g;
     const int N = g.N;
-    const unsigned blocks = (unsigned)(N / kC);
+    // split the planes in two when that fills the last wave of CTAs better (one CTA per SM)
+    const int items = N / kC, sms = p->sm_count;
+    const double r1 = (double)((items + sms - 1) / sms), r2 = 0.5 * (double)((2 * items + sms - 1) / sms);
+    const int ksplit = (g.Nw >= 2 && r2 < 0.95 * r1) ? 2 : 1;
+    if (ksplit > 1 && zero_first) RICK_CUDA(cudaMemsetAsync(image, 0, sizeof(double) * (size_t)N * N, st));
+    const dim3 blocks((unsigned)items, (unsigned)ksplit);
     const size_t smem = colfft_smem_bytes(N);
     const float2* planes = (const float2*)grid;
     const float2* tw = (const float2*)p->colfft_tw;
