@@ -12,7 +12,7 @@
 // The transformed planes are never written back: the column pass of a 2-D FFT (read + write of the
 // mesh) and the K5 sweep (another read) collapse into one read.
 //
-// Phase: w_k * nm1 reduced to [-1/2, 1/2] turns in fp64 (nm1 per pixel kept in shared memory), then the
+// Phase: w_k * nm1 reduced to [-1/2, 1/2] turns in fp64 (nm1 of a thread's pixels kept in registers), then the
 // hardware sine / cosine in fp32 on the reduced argument (abs error < 5e-7, the precision of the fp32
 // planes themselves); the product in fp32, the plane sum in fp64.
 #include "rick_internal.cuh"
@@ -161,10 +161,20 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
     float2* buf0 = reinterpret_cast<float2*>(smem_raw);
     float2* buf1 = buf0 + buf_elems;
     float2* tw = buf1 + buf_elems;                    // [N]
-    double* nm1_s = reinterpret_cast<double*>(tw + N);   // [n_slots], indexed like the data (unpadded)
     const int tid = threadIdx.x;
     const int p0 = blockIdx.x * kC;
     constexpr int per_thread = n_slots / kT;          // outputs owned by a thread: 2 .. 16
+    // Ownership: with a third pass (R3 > 1) a thread keeps the R3 outputs of each of its last-pass
+    // butterflies (entry e = bi R3 + u: butterfly w = bi kT + tid, sub-block B = w / kC, column c = w % kC,
+    // slot (B R3 + u) kC + c) -- they go from registers straight into the screen, never back to shared
+    // memory; without one (N = 256) entry e is slot e kT + tid, read back from shared memory.
+    auto owned_slot = [&](int e) {
+        if (R3 > 1) {
+            const int bi = e / R3, u = e % R3, w = bi * kT + tid;
+            return ((w / kC) * R3 + u) * kC + (w % kC);
+        }
+        return e * kT + tid;
+    };
 
     auto issue = [&](int k, float2* buf) {
         const float2* src = planes + (size_t)k * N * N + p0;
@@ -183,16 +193,23 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
     if (k_lo >= k_hi) return;
     issue(k_lo, buf0);
     for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
+    double acc[per_thread], nm1r[per_thread];         // plane sum and n - 1 of the owned pixels
+#pragma unroll
     for (int e = 0; e < per_thread; ++e) {
-        const int idx = e * kT + tid;
+        const int idx = owned_slot(e);
         const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
         const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
         const double r2 = l * l + m * m;
-        nm1_s[idx] = -r2 / (1.0 + sqrt(1.0 - r2));
+        nm1r[e] = -r2 / (1.0 + sqrt(1.0 - r2));
+        acc[e] = 0.0;
     }
-    double acc[16];                                   // per_thread <= 16 (N <= 2048)
-#pragma unroll
-    for (int e = 0; e < 16; ++e) acc[e] = 0.0;
+    auto screen_add = [&](int e, float2 v, double wk) {
+        double t = wk * nm1r[e];
+        t -= rint(t);                                          // [-1/2, 1/2] turns
+        float sn, cs;
+        __sincosf(6.283185307179586f * (float)t, &sn, &cs);    // MUFU on [-pi, pi]: abs error < 5e-7
+        acc[e] += (double)(cs * v.x - sn * v.y);
+    };
 
     for (int k = k_lo; k < k_hi; ++k) {
         const int par = (k - k_lo) & 1;
@@ -205,39 +222,38 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         __syncthreads();
         dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid);
         __syncthreads();
-        if (R3 > 1) {
-            dif_pass<LOG2N, R3, LOG2N - 8>(buf, tw, tid);
-            __syncthreads();
-        }
         const double wk = g.w_min + ((double)k + 0.5) * g.dw;
+        if (R3 > 1) {
+            // last pass (sub-length R3, no twiddles) fused with the screen: outputs stay in registers
 #pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            if (e < per_thread) {
-                const int idx = e * kT + tid;
-                const float2 v = buf[padded(idx)];
-                double t = wk * nm1_s[idx];
-                t -= rint(t);                                  // [-1/2, 1/2] turns
-                float sn, cs;
-                __sincosf(6.283185307179586f * (float)t, &sn, &cs);   // MUFU on [-pi, pi]: abs error < 5e-7
-                acc[e] += (double)(cs * v.x - sn * v.y);
+            for (int bi = 0; bi < per_thread / R3; ++bi) {
+                const int w = bi * kT + tid;
+                const int pb = padded((w / kC) * (R3 * kC) + (w % kC));   // R3 * kC <= 32: one padding group
+                float2 v[R3];
+#pragma unroll
+                for (int t = 0; t < R3; ++t) v[t] = buf[pb + t * kC];
+                dft<R3>(v);
+#pragma unroll
+                for (int u = 0; u < R3; ++u) screen_add(bi * R3 + u, v[u], wk);
             }
+        } else {
+#pragma unroll
+            for (int e = 0; e < per_thread; ++e) screen_add(e, buf[padded(e * kT + tid)], wk);
         }
         __syncthreads();                              // buf is free for plane k + 2
     }
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-        if (e < per_thread) {
-            const int idx = e * kT + tid;
-            const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
-            const double sg = ((p + q) & 1) ? -1.0 : 1.0;
-            double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
-            const size_t o = (size_t)q * N + p;
-            if (gridDim.y > 1) {
-                atomicAdd(image + o, out);       // two addends onto a zeroed or given image: order-independent
-            } else {
-                if (accumulate) out += image[o];
-                image[o] = out;
-            }
+    for (int e = 0; e < per_thread; ++e) {
+        const int idx = owned_slot(e);
+        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
+        const double sg = ((p + q) & 1) ? -1.0 : 1.0;
+        double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
+        const size_t o = (size_t)q * N + p;
+        if (gridDim.y > 1) {
+            atomicAdd(image + o, out);       // two addends onto a zeroed or given image: order-independent
+        } else {
+            if (accumulate) out += image[o];
+            image[o] = out;
         }
     }
 }
@@ -245,7 +261,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 size_t colfft_smem_bytes(int N) {
     const int n_slots = N * kC;
     const size_t buf = (size_t)(n_slots + ((n_slots >> kPadShift) << 2)) * sizeof(float2);
-    return 2 * buf + (size_t)N * sizeof(float2) + (size_t)n_slots * sizeof(double);
+    return 2 * buf + (size_t)N * sizeof(float2);
 }
 
 }  // namespace
