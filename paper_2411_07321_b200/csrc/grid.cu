@@ -229,7 +229,7 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 
-template <int S, int RB, int L>
+template <int S, int RB, int L, int NBUF>
 __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                          const uint2* __restrict__ ga, const float2* __restrict__ gb,
                                                          const float2* __restrict__ gc, float2* __restrict__ grid,
@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 
     // stage st of every thread's range -> buffer st & 1 (16 lanes copy one thread's 16 * PPT bytes per stream)
     auto issue = [&](int st) {
-        uint4* buf = stage + (st & 1) * (3 * NP);
+        uint4* buf = stage + (st % NBUF) * (3 * NP);
 #pragma unroll 4
         for (int q = tid; q < NP; q += kRunThreads) {
             const int t = q / PPT, piece = q % PPT;
@@ -279,8 +279,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
         uint32_t cij = 0xFFFFFFFFu, ck = 0;
 
         auto flush = [&]() {
-            const int ci = (int)(cij & 0xFFFFu), cj = (int)(cij >> 16);
-            const int iw = (ci - h) & ~1;
+            const int iw = (int)(cij & 0xFFFFu), cj = (int)(cij >> 16);   // cij: window column | j0 << 16
             float2* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)iw;
             const bool edge = iw + W > (int)N;      // the zero column would fall past the row (i0 = N-1-h)
 #pragma unroll
@@ -298,9 +297,12 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
         };
 
         auto one = [&](uint32_t ij, uint32_t k, float dx, float dy, float vr, float vi) {
-            if (ij != cij || k != ck) {
+            // the even-aligned window of a cell: cells i0, i0 + 1 with i0 - h even share it, so a run of
+            // visibilities on two neighbouring cells accumulates into the same registers
+            const uint32_t wij = (ij - (uint32_t)h) & ~1u;          // i0 >= h: no borrow into j0
+            if (wij != cij || k != ck) {
                 if (cij != 0xFFFFFFFFu) flush();
-                cij = ij; ck = k;
+                cij = wij; ck = k;
             }
             float t[S], gx[W], gy[S];
             taps_f32<S, true>(gy, dy, c2, tc);
@@ -329,13 +331,18 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
         issue(0);
 #pragma unroll 1
         for (int st = 0; st < n_stage; ++st) {
-            if (st + 1 < n_stage) issue(st + 1);
-            else asm volatile("cp.async.commit_group;" ::: "memory");
-            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            if (NBUF == 2) {
+                if (st + 1 < n_stage) issue(st + 1);
+                else asm volatile("cp.async.commit_group;" ::: "memory");
+                asm volatile("cp.async.wait_group 1;" ::: "memory");
+            } else {
+                if (st > 0) issue(st);
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+            }
             __syncthreads();
             const long long left = n - (first + (long long)st * L);
             const int cnt = left >= L ? L : (left > 0 ? (int)left : 0);
-            const uint4* my = stage + (st & 1) * (3 * NP) + tid * PPT;
+            const uint4* my = stage + (st % NBUF) * (3 * NP) + tid * PPT;
 #pragma unroll 1
             for (int i = 0; i < cnt; i += 2) {
                 const int piece = (i >> 1) ^ sw;
@@ -355,10 +362,14 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 template <int S, int RB>
 int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
     constexpr int L = 16;                                   // records per thread and stage
-    constexpr int smem = 2 * 3 * kRunThreads * (L / 2) * 16;   // two buffers of three streams: 96 KB
+#ifndef RICK_GRID_NBUF
+#define RICK_GRID_NBUF 2
+#endif
+    constexpr int NBUF = RICK_GRID_NBUF;
+    constexpr int smem = NBUF * 3 * kRunThreads * (L / 2) * 16;   // NBUF buffers of three streams, 48 KB each
     static bool attr_done = false;
     if (!attr_done) {
-        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return RICK_ECUDA;
         attr_done = true;
     }
@@ -374,7 +385,7 @@ int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
     n_stage = n_stage < 2 ? 2 : (n_stage > 16 ? 16 : n_stage);
     const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
-    k_grid_rec<S, RB, L><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
+    k_grid_rec<S, RB, L, NBUF><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
                                                            (float2*)grid, n_stage);
     return RICK_OK;
 }
