@@ -117,12 +117,6 @@ int rick_bin(rick_plan* plan, long long M, const float* u, const float* v, const
              float* weight_s, unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out,
              void* workspace, size_t workspace_bytes, long long* n_kept_dev, void* stream);
 
-/* Optional: start clearing the mesh now, on a stream of the plan's own, ordered after the work already
- * queued on `stream`; the next rick_grid(plan, grid, zero_first != 0, ...) on the same mesh then waits for
- * that clear instead of clearing itself.  Called before rick_bin it overlaps the HBM-bound clear with
- * the sort.  The mesh must not be touched between this call and that rick_grid. */
-int rick_grid_prezero(rick_plan* plan, void* grid, void* stream);
-
 /* Gridding, Eq. 3 [D6], of the visibilities bound by the last rick_bin into
  * grid[Nw][N][N] (device, dtype of the plan, caller-owned).  zero_first != 0 clears the mesh first;
  * zero_first == 0 accumulates onto its contents (chunked inputs).

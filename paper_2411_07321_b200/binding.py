@@ -22,7 +22,7 @@ _lib = None
 EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
     "rick_plan_sort_layout", "rick_plan_set_fusion",
-    "rick_bin", "rick_grid", "rick_grid_prezero", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
+    "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
 
@@ -65,7 +65,6 @@ def lib():
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
-        L.rick_grid_prezero.argtypes = [vp, vp, vp]
         L.rick_fft_planes.argtypes = [vp, vp, vp, sz, vp]
         L.rick_wcorrect_accumulate.argtypes = [vp, vp, vp, i, vp]
         L.rick_image.argtypes = [vp, vp, vp, i, vp]
@@ -168,12 +167,6 @@ def rick_grid(plan: int, grid: torch.Tensor, zero_first: bool = True, stream=Non
     _check(lib().rick_grid(plan, _ptr(grid), 1 if zero_first else 0, _stream(stream)), "rick_grid")
 
 
-def rick_grid_prezero(plan: int, grid: torch.Tensor, stream=None) -> None:
-    if not (grid.is_cuda and grid.is_contiguous()):
-        raise RickError("grid: expected a contiguous CUDA tensor")
-    _check(lib().rick_grid_prezero(plan, _ptr(grid), _stream(stream)), "rick_grid_prezero")
-
-
 def rick_fft_planes(plan: int, grid: torch.Tensor, fft_work: Optional[torch.Tensor], stream=None) -> None:
     nbytes = 0 if fft_work is None else fft_work.numel() * fft_work.element_size()
     _check(lib().rick_fft_planes(plan, _ptr(grid), _ptr(fft_work), nbytes, _stream(stream)), "rick_fft_planes")
@@ -274,9 +267,7 @@ class Imager:
         rick_wcorrect_accumulate(self.plan, self.grid, self.image, zero_first)
 
     def run(self, u, v, w, vis, weight) -> torch.Tensor:
-        """(mesh clear overlapped with) bin -> grid -> FFT -> w-correct on device-resident inputs; returns
-        the device image."""
-        rick_grid_prezero(self.plan, self.grid)
+        """bin -> grid -> FFT -> w-correct on device-resident inputs; returns the device image."""
         self.bin(u, v, w, vis, weight)
         self.grid_(True)
         self.fft()

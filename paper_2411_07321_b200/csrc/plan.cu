@@ -183,12 +183,6 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
             return RICK_ECUDA;
         }
     }
-    if (cudaStreamCreateWithFlags(&p->zero_stream, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_zero_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_zero_done, cudaEventDisableTiming) != cudaSuccess) {
-        rick_plan_destroy(p);
-        return RICK_ECUDA;
-    }
     *out = p;
     return RICK_OK;
 }
@@ -237,9 +231,6 @@ int rick_plan_destroy(rick_plan* p) {
     destroy_fft(p);
     if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
     if (p->colfft_tw) cudaFree(p->colfft_tw);
-    if (p->zero_stream) { cudaStreamSynchronize(p->zero_stream); cudaStreamDestroy(p->zero_stream); }
-    if (p->ev_zero_fork) cudaEventDestroy(p->ev_zero_fork);
-    if (p->ev_zero_done) cudaEventDestroy(p->ev_zero_done);
     for (int i = 0; i < RICK_T_COUNT; ++i) {
         if (p->ev_start[i]) cudaEventDestroy(p->ev_start[i]);
         if (p->ev_stop[i]) cudaEventDestroy(p->ev_stop[i]);
@@ -262,30 +253,11 @@ int rick_bin(rick_plan* p, long long M, const float* u, const float* v, const fl
                          key_out, perm_out, bin_start_out, workspace, workspace_bytes, n_kept_dev, st);
 }
 
-int rick_grid_prezero(rick_plan* p, void* grid, void* stream) {
-    if (!p || !grid) return RICK_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    const size_t cell = (p->dtype == RICK_C128) ? 16 : 8;
-    // fork: the clear starts once everything already queued on `stream` (earlier readers of the mesh) is done
-    RICK_CUDA(cudaEventRecord(p->ev_zero_fork, st));
-    RICK_CUDA(cudaStreamWaitEvent(p->zero_stream, p->ev_zero_fork, 0));
-    {
-        StageTimer tz(p, RICK_T_ZERO, p->zero_stream);
-        RICK_CUDA(cudaMemsetAsync(grid, 0, cell * (size_t)p->g.Nw * (size_t)p->g.N * (size_t)p->g.N, p->zero_stream));
-    }
-    RICK_CUDA(cudaEventRecord(p->ev_zero_done, p->zero_stream));
-    p->prezeroed_grid = grid;
-    return RICK_OK;
-}
-
 int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
     if (!p || !grid) return RICK_EINVAL;
     if (!p->bound) return RICK_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (zero_first && p->prezeroed_grid == grid) {      // join the clear started by rick_grid_prezero
-        RICK_CUDA(cudaStreamWaitEvent(st, p->ev_zero_done, 0));
-        p->prezeroed_grid = NULL;
-    } else if (zero_first) {
+    if (zero_first) {
         StageTimer tz(p, RICK_T_ZERO, st);
         const size_t cell = (p->dtype == RICK_C128) ? 16 : 8;
         RICK_CUDA(cudaMemsetAsync(grid, 0, cell * (size_t)p->g.Nw * (size_t)p->g.N * (size_t)p->g.N, st));
@@ -358,9 +330,7 @@ int rick_image_from_host(rick_plan* p, long long M, const float* u_h, const floa
         RICK_CUDA(cudaMemcpyAsync(d->vis, vis_h, 8 * m, cudaMemcpyHostToDevice, st));
         RICK_CUDA(cudaMemcpyAsync(d->weight, weight_h, 4 * m, cudaMemcpyHostToDevice, st));
     }
-    int rc = rick_grid_prezero(p, d->grid, stream);
-    if (rc != RICK_OK) return rc;
-    rc = rick_bin(p, M, d->u, d->v, d->w, d->vis, d->weight, d->u_s, d->v_s, d->w_s, d->vis_s, d->weight_s,
+    int rc = rick_bin(p, M, d->u, d->v, d->w, d->vis, d->weight, d->u_s, d->v_s, d->w_s, d->vis_s, d->weight_s,
                       NULL, NULL, NULL, d->workspace, d->workspace_bytes, d->n_kept, stream);
     if (rc != RICK_OK) return rc;
     if ((rc = rick_grid(p, d->grid, 1, stream)) != RICK_OK) return rc;

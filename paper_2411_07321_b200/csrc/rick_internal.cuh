@@ -59,10 +59,6 @@ struct rick_plan {
     //   a = (i0 | j0 << 16, k), b = (i0 - x, j0 - y) in fp32, c = +-weight * (re, im)
     const uint2* grec_a;
     const float2 *grec_b, *grec_c;
-    // mesh zeroing overlapped with rick_bin (rick_grid_prezero): side stream + fork/join events
-    cudaStream_t zero_stream;
-    cudaEvent_t ev_zero_fork, ev_zero_done;
-    void* prezeroed_grid;
     // stage timing
     cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
     bool ev_valid[RICK_T_COUNT];
