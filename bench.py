@@ -48,6 +48,22 @@ def _traffic(kernel: str):
         return None
 
 
+def max_over_ranks(x: float, dist, device) -> float:
+    """Replicas-only multi-GPU accounting: a timed quantity of the job is the slowest
+    rank's; there is no data-path collective, this all-reduce of one scalar is the only exchange."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(per_rank_units: int, world: int, ms_per_step: float) -> float:
+    """Whole-job throughput: every rank images its own replica of the workload (weak scaling)."""
+    return world * per_rank_units / (ms_per_step * 1e-3)
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -232,13 +248,11 @@ def main():
     launches = im.launches() - l0
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
+    ms = max_over_ranks(ms, dist, dev)
     if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.barrier()
-        ms = float(t.item())
     ms_per_step = ms / args.steps
-    value = world * M / (ms_per_step * 1e-3)
+    value = job_value(M, world, ms_per_step)
 
     # per-stage CUDA-event times (events recorded by the library on the launch stream), same workload
     per = {k: [] for k in B.RICK_T_NAMES}
@@ -299,10 +313,7 @@ def main():
             im.run_from_host(*host, out)
         torch.cuda.synchronize()
         e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-        if dist is not None:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = max_over_ranks(e2e_s, dist, dev)
         e2e = {"value": world * M / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
                "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps}
 
