@@ -419,7 +419,7 @@ int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st) {
         case 3:  if (f64) launch_runs<double, 3, 3>(p, grid, st);  else rc = launch_rec<3, 3>(p, grid, st); break;
         case 5:  if (f64) launch_runs<double, 5, 5>(p, grid, st);  else rc = launch_rec<5, 5>(p, grid, st); break;
         case 7:  if (f64) launch_runs<double, 7, 4>(p, grid, st);  else rc = launch_rec<7, 7>(p, grid, st); break;
-        case 9:  if (f64) launch_runs<double, 9, 3>(p, grid, st);  else rc = launch_rec<9, 5>(p, grid, st); break;
+        case 9:  if (f64) launch_runs<double, 9, 3>(p, grid, st);  else rc = launch_rec<9, 9>(p, grid, st); break;
         case 11: if (f64) launch_runs<double, 11, 2>(p, grid, st); else rc = launch_rec<11, 4>(p, grid, st); break;
         case 13: if (f64) launch_runs<double, 13, 2>(p, grid, st); else rc = launch_rec<13, 3>(p, grid, st); break;
         case 15: if (f64) launch_runs<double, 15, 2>(p, grid, st); else rc = launch_rec<15, 3>(p, grid, st); break;
