@@ -38,8 +38,29 @@ namespace {
 typedef std::complex<double> cplx;
 const double kPi = 3.14159265358979323846264338327950288;
 
+// Gridding kernel family, selected process-wide by rick_oracle_set_kernel (the Python front end sets it
+// from the Plan before every call):  0 = truncated Gaussian (BASELINE.json north_star; D6),
+// 1 = Kaiser-Bessel (the kernel of the paper's own tests; D6-KB of DESIGN.md).
+int g_kernel_kind = 0;
+double g_kernel_beta = 0.0;
+
+// Modified Bessel function of the first kind, order 0, by its power series
+//   I0(x) = sum_k (x^2 / 4)^k / (k!)^2      (all terms positive: no cancellation)
+double bessel_i0(double x) {
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+
 struct Geometry {
     int N, Nw, S, h;
+    int kernel;      // 0 Gaussian, 1 Kaiser-Bessel
+    double beta, i0_beta;   // KB shape parameter and I0(beta)
     double sigma, w_min, w_max, dl;
     double s;        // D2: (double)N * dl, one rounded multiply
     double inv_dw;   // D3: (double)Nw / (w_max - w_min)
@@ -50,6 +71,8 @@ Geometry make_geometry(int N, int Nw, int S, double sigma, double w_min, double 
     Geometry g;
     g.N = N; g.Nw = Nw; g.S = S; g.h = (S - 1) / 2;
     g.sigma = sigma; g.w_min = w_min; g.w_max = w_max; g.dl = dl;
+    g.kernel = g_kernel_kind; g.beta = g_kernel_beta;
+    g.i0_beta = g.kernel == 1 ? bessel_i0(g.beta) : 1.0;
     g.s = (double)N * dl;
     g.inv_dw = (double)Nw / (w_max - w_min);
     g.T = N / 32;
@@ -81,8 +104,18 @@ bool locate(const Geometry& g, float u, float v, float w, float vre, float vim, 
     return true;
 }
 
-// D6 tap: un-normalised Gaussian, sigma in cells.
-inline double tap(double d, double sigma) { return std::exp(-(d * d) / (2.0 * sigma * sigma)); }
+// D6 tap.  Gaussian: g(d) = exp(-d^2 / 2 sigma^2), un-normalised, sigma in cells.
+// D6-KB: g(d) = I0(beta sqrt(1 - (d / a_t)^2)) / I0(beta) for |d| <= a_t = h + 1/2 (the footprint offsets
+// satisfy -a_t < d <= a_t), the Kaiser-Bessel window of full width 2 a_t = S cells.
+inline double tap(double d, const Geometry& g) {
+    if (g.kernel == 1) {
+        const double a_t = (double)g.h + 0.5;
+        const double r = d / a_t;
+        const double arg = 1.0 - r * r;
+        return bessel_i0(g.beta * std::sqrt(arg > 0.0 ? arg : 0.0)) / g.i0_beta;
+    }
+    return std::exp(-(d * d) / (2.0 * g.sigma * g.sigma));
+}
 
 // ---- own radix-2 FFT (sign +, unnormalised), used for D7 -------------------------------------
 void fft1d_inverse(cplx* a, int n) {
@@ -139,8 +172,24 @@ inline double nm1_of(double l, double m) {
 
 // D8 1-D taper table: t[p] = c0 exp(-2 pi^2 sigma^2 nu_p^2), nu_p = (p - N/2)/N,
 // c0 = sigma sqrt(2 pi) erf(a_t / (sigma sqrt 2)), a_t = h + 1/2 (integral of the truncated kernel).
+// D8-KB: the exact transform of the compactly supported Kaiser-Bessel window,
+//   t(nu) = int_{-a_t}^{a_t} g(d) e^{-2 pi i nu d} dd = (2 a_t / I0(beta)) sinh(z) / z,  z = sqrt(beta^2 - (2 pi a_t nu)^2)
+// (sin(z') / z' with z' = sqrt((2 pi a_t nu)^2 - beta^2) beyond the main lobe; 1 at z = 0).
 void taper_table(const Geometry& g, double* t) {
     const double a_t = (double)g.h + 0.5;
+    if (g.kernel == 1) {
+        for (int p = 0; p < g.N; ++p) {
+            const double nu = (double)(p - g.N / 2) / (double)g.N;
+            const double y = 2.0 * kPi * a_t * nu;
+            const double z2 = g.beta * g.beta - y * y;
+            double sc;
+            if (z2 > 1e-24) { const double z = std::sqrt(z2); sc = std::sinh(z) / z; }
+            else if (z2 < -1e-24) { const double z = std::sqrt(-z2); sc = std::sin(z) / z; }
+            else sc = 1.0;
+            t[p] = 2.0 * a_t * sc / g.i0_beta;
+        }
+        return;
+    }
     const double c0 = g.sigma * std::sqrt(2.0 * kPi) * std::erf(a_t / (g.sigma * std::sqrt(2.0)));
     for (int p = 0; p < g.N; ++p) {
         const double nu = (double)(p - g.N / 2) / (double)g.N;
@@ -170,10 +219,10 @@ void grid_plane(const Geometry& g, const std::vector<uint32_t>& list, const floa
             for (int b = -h; b <= h; ++b) {
                 const long j = j0 + b;
                 if (j < j_lo || j >= j_hi) continue;
-                const double gy = tap((double)j - y, g.sigma);
+                const double gy = tap((double)j - y, g);
                 for (int a = -h; a <= h; ++a) {
                     const long i = i0 + a;
-                    const double gx = tap((double)i - x, g.sigma);
+                    const double gx = tap((double)i - x, g);
                     plane[(size_t)j * N + i] += val * (gx * gy);
                 }
             }
@@ -213,6 +262,15 @@ int rick_oracle_threads() {
     return 1;
 #endif
 }
+
+// Select the gridding kernel used by every later call: kind 0 Gaussian (sigma of each call), kind 1
+// Kaiser-Bessel with shape parameter beta (sigma is then ignored).
+void rick_oracle_set_kernel(int kind, double beta) {
+    g_kernel_kind = kind == 1 ? 1 : 0;
+    g_kernel_beta = beta;
+}
+
+double rick_oracle_bessel_i0(double x) { return bessel_i0(x); }
 
 void rick_oracle_set_threads(int n) {
 #ifdef _OPENMP

@@ -38,6 +38,9 @@ def lib():
         geo = [C.c_int, C.c_int, C.c_int]
         L.rick_oracle_threads.restype = C.c_int
         L.rick_oracle_set_threads.argtypes = [C.c_int]
+        L.rick_oracle_set_kernel.argtypes = [C.c_int, C.c_double]
+        L.rick_oracle_bessel_i0.restype = C.c_double
+        L.rick_oracle_bessel_i0.argtypes = [C.c_double]
         L.rick_oracle_keys.restype = C.c_longlong
         L.rick_oracle_keys.argtypes = geo + [C.c_double, C.c_double, C.c_double, C.c_longlong,
                                              f32p, f32p, f32p, f32p, f32p, u32p, i32p, i32p, i32p]
@@ -75,6 +78,8 @@ class Plan:
     w_min: float
     w_max: float
     dl: float
+    kernel: str = "gauss"      # "gauss" (D6, BASELINE.json north_star) or "kb" (D6-KB, the paper's kernel)
+    beta: float = 0.0          # Kaiser-Bessel shape parameter (kernel == "kb")
 
     @property
     def T(self) -> int:
@@ -83,6 +88,17 @@ class Plan:
     @property
     def n_bins(self) -> int:
         return self.Nw * self.T * self.T
+
+
+def _select(kernel: str = "gauss", beta: float = 0.0) -> None:
+    """Set the oracle's process-wide gridding kernel (done before every call that grids or tapers)."""
+    if kernel not in ("gauss", "kb"):
+        raise ValueError(kernel)
+    lib().rick_oracle_set_kernel(1 if kernel == "kb" else 0, float(beta))
+
+
+def bessel_i0(x: float) -> float:
+    return float(lib().rick_oracle_bessel_i0(float(x)))
 
 
 def _inputs(u, v, w, vis, wt):
@@ -149,6 +165,7 @@ def grid(plan: Plan, u, v, w, vis, wt) -> np.ndarray:
     """-> complex128 [Nw, N, N] (D6; un-modulated mesh)."""
     u, v, w, vis, wt, M = _inputs(u, v, w, vis, wt)
     g = np.empty((plan.Nw, plan.N, plan.N), np.complex128)
+    _select(plan.kernel, plan.beta)
     lib().rick_oracle_grid(plan.N, plan.Nw, plan.support, plan.sigma, plan.w_min, plan.w_max, plan.dl, M,
                            _p(u, C.c_float), _p(v, C.c_float), _p(w, C.c_float),
                            _p(vis.view(np.float32), C.c_float), _p(wt, C.c_float),
@@ -174,8 +191,9 @@ def plane_transform_literal(plane: np.ndarray) -> np.ndarray:
     return out
 
 
-def taper(N: int, support: int, sigma: float) -> np.ndarray:
+def taper(N: int, support: int, sigma: float, kernel: str = "gauss", beta: float = 0.0) -> np.ndarray:
     t = np.empty(N, np.float64)
+    _select(kernel, beta)
     lib().rick_oracle_taper(N, support, sigma, _p(t, C.c_double))
     return t
 
@@ -192,6 +210,7 @@ def wcorrect(plan: Plan, planes: np.ndarray) -> np.ndarray:
     P = np.ascontiguousarray(planes, dtype=np.complex128)
     assert P.shape == (plan.Nw, plan.N, plan.N)
     img = np.empty((plan.N, plan.N), np.float64)
+    _select(plan.kernel, plan.beta)
     lib().rick_oracle_wcorrect(plan.N, plan.Nw, plan.support, plan.sigma, plan.w_min, plan.w_max, plan.dl,
                                _p(P.view(np.float64), C.c_double), _p(img, C.c_double))
     return img
@@ -202,6 +221,7 @@ def image(plan: Plan, u, v, w, vis, wt, return_timing: bool = False):
     u, v, w, vis, wt, M = _inputs(u, v, w, vis, wt)
     img = np.empty((plan.N, plan.N), np.float64)
     st = np.zeros(4, np.float64)
+    _select(plan.kernel, plan.beta)
     n = lib().rick_oracle_image(plan.N, plan.Nw, plan.support, plan.sigma, plan.w_min, plan.w_max, plan.dl, M,
                                 _p(u, C.c_float), _p(v, C.c_float), _p(w, C.c_float),
                                 _p(vis.view(np.float32), C.c_float), _p(wt, C.c_float),

@@ -502,3 +502,84 @@ def test_dropped_visibilities_do_not_contribute():
     e = np.zeros(0, np.float32)
     z = O.image(plan, e, e, e, np.zeros(0, np.complex64), e)
     assert np.all(z == 0.0)
+
+
+# ------------------------------------------------------------------------------------------------
+# Kaiser-Bessel kernel (D6-KB: the kernel of the paper's own tests)
+# ------------------------------------------------------------------------------------------------
+
+KB = dict(kernel="kb", beta=2.34 * 7)
+
+
+def _kb(d, a_t, beta):
+    from scipy import special
+    return special.i0(beta * np.sqrt(np.clip(1.0 - (np.asarray(d, np.float64) / a_t) ** 2, 0.0, None))) / special.i0(beta)
+
+
+def test_kb_bessel_series_against_scipy():
+    from scipy import special
+    for x in (0.0, 1e-3, 0.7, 3.75, 9.0, 16.38, 21.06, 40.0):
+        assert abs(O.bessel_i0(x) / special.i0(x) - 1.0) < 5e-15
+
+
+@pytest.mark.parametrize("S,beta", [(7, 2.34 * 7), (9, 2.34 * 9), (5, 9.0)])
+def test_kb_footprint_taper_and_tap_sum(S, beta):
+    """Single-visibility footprint against the window typed with scipy's I0; the taper against numerical
+    integration of the window (it is its exact transform); tap sums average to the taper's centre value."""
+    h, a_t = (S - 1) // 2, (S - 1) // 2 + 0.5
+    plan = O.Plan(N=64, Nw=2, support=S, sigma=1.0, w_min=-1.0, w_max=1.0, dl=0.3 / 64, kernel="kb", beta=beta)
+    s = plan.N * plan.dl
+    u = np.array([3.3 / s], np.float32)
+    v = np.array([-7.8 / s], np.float32)
+    g = O.grid(plan, u, v, np.array([0.5], np.float32), np.array([1.5 - 0.25j], np.complex64), np.array([0.75], np.float32))
+    x, y = float(u[0]) * s + 32, float(v[0]) * s + 32
+    i0, j0 = int(math.floor(x + 0.5)), int(math.floor(y + 0.5))
+    exp = np.zeros((2, 64, 64), np.complex128)
+    ii, jj = np.arange(i0 - h, i0 + h + 1), np.arange(j0 - h, j0 + h + 1)
+    exp[1, j0 - h:j0 + h + 1, i0 - h:i0 + h + 1] = (1.5 - 0.25j) * 0.75 * np.outer(_kb(jj - y, a_t, beta), _kb(ii - x, a_t, beta))
+    np.testing.assert_allclose(g, exp, rtol=1e-12, atol=1e-15)
+    # the Gaussian oracle is untouched by the selection (state is set per call)
+    g0 = O.grid(O.Plan(N=64, Nw=2, support=S, sigma=1.0, w_min=-1.0, w_max=1.0, dl=0.3 / 64), u, v,
+                np.array([0.5], np.float32), np.array([1.0], np.complex64), np.array([1.0], np.float32))
+    assert abs(g0[1, j0, i0] - math.exp(-((i0 - x) ** 2 + (j0 - y) ** 2) / 2.0)) < 1e-14
+    N = 256
+    t = O.taper(N, S, 1.0, "kb", beta)
+    for p in (N // 2, N // 2 + 37, 11, 0):
+        nu = (p - N // 2) / N
+        val = integrate.quad(lambda d: float(_kb(d, a_t, beta)) * math.cos(2 * math.pi * nu * d), -a_t, a_t,
+                             epsabs=1e-13, epsrel=1e-13, limit=400)[0]
+        assert abs(val - t[p]) < 1e-11 * t[N // 2]
+    rng = np.random.default_rng(8)
+    off = rng.uniform(-0.5, 0.5, 20000)
+    sums = _kb(off[:, None] + np.arange(-h, h + 1)[None, :], a_t, beta).sum(1)
+    assert abs(sums.mean() - t[N // 2]) < 5e-3 * t[N // 2]
+
+
+def test_kb_closed_forms_and_bruteforce():
+    """Same end-to-end pins as for the Gaussian: phase-centre source -> weight sum; against the exact dirty
+    image on a tiny wide-field case (the Kaiser-Bessel window aliases less: a tighter bound holds)."""
+    rng = np.random.default_rng(31)
+    plan = O.Plan(N=128, Nw=8, support=7, sigma=1.0, w_min=-300.0, w_max=300.0, dl=0.2 / 128, **KB)
+    M = 5000
+    u, v, w = _rand_vis(rng, M, plan.N, 0.2, -300, 300)
+    img, n_kept, _ = O.image(plan, u, v, w, np.ones(M, np.complex64), np.ones(M, np.float32), return_timing=True)
+    assert n_kept == M and np.unravel_index(np.argmax(img), img.shape) == (64, 64)
+    assert abs(img[64, 64] / M - 1.0) <= 1e-4
+    N, fov = 64, 0.6
+    plan = O.Plan(N=N, Nw=8, support=7, sigma=1.0, w_min=-150.0, w_max=150.0, dl=fov / N, **KB)
+    M = 400
+    rng = np.random.default_rng(41)
+    u, v, w = _rand_vis(rng, M, N, fov, -150, 150, margin=5.0)
+    w = _snap_w(plan, w)
+    vis = np.zeros(M, np.complex64)
+    for amp, l0, m0 in [(1.0, 0.11, -0.07), (0.7, -0.13, 0.12), (1.6, 0.02, 0.05)]:
+        vis = vis + _point_vis(u, v, w, l0, m0, amp)
+    wt = rng.uniform(0.5, 1.0, M).astype(np.float32)
+    img = O.image(plan, u, v, w, vis, wt)
+    ref = O.direct_dft(plan, u, v, w, vis, wt)
+    inner = slice(N // 4, 3 * N // 4)
+    err = np.abs(img - ref)[inner, inner].max() / np.abs(ref[inner, inner]).max()
+    gauss = O.image(O.Plan(N=N, Nw=8, support=7, sigma=1.0, w_min=-150.0, w_max=150.0, dl=fov / N), u, v, w, vis, wt)
+    err_g = np.abs(gauss - ref)[inner, inner].max() / np.abs(ref[inner, inner]).max()
+    print(f"KB vs exact {err:.2e}; Gaussian vs exact {err_g:.2e}")
+    assert err <= 1e-3 and err < err_g
