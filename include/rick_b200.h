@@ -56,6 +56,9 @@ typedef enum {
 
 typedef enum { RICK_C64 = 0, RICK_C128 = 1 } rick_dtype;
 
+/* gridding kernel families of rick_plan_set_kernel */
+typedef enum { RICK_KERNEL_GAUSS = 0, RICK_KERNEL_KB = 1 } rick_kernel;
+
 /* stage indices of rick_get_timings */
 enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_WCORRECT = 4,
        RICK_T_IMAGE = 5,
@@ -76,6 +79,15 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
 
 /* Select the mesh dtype and (re)build the cuFFT plan for it.  Host-synchronous. */
 int rick_plan_set_dtype(rick_plan* plan, int dtype);
+
+/* Gridding kernel G of Eq. 3.  Default: the separable truncated Gaussian of rick_plan_create
+ * (BASELINE.json north_star) [D6].  RICK_KERNEL_KB selects the separable Kaiser-Bessel window the paper's
+ * own tests use: g(d) = I0(beta sqrt(1 - (d / a_t)^2)) / I0(beta), |d| <= a_t = support / 2, with
+ * shape parameter `param` = beta > 0 (sigma is then unused), and the taper table becomes its exact
+ * transform 2 a_t sinh(z) / (z I0(beta)), z = sqrt(beta^2 - (2 pi a_t nu)^2)  [D6-KB, D8-KB].
+ * Host-synchronous (rebuilds the taper and tap tables); call before rick_grid / rick_wcorrect_accumulate.
+ * Errors: RICK_EINVAL (unknown kind, beta <= 0 or > 64), RICK_ENOMEM, RICK_ECUDA. */
+int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
 
 /* Fused column transform (optional; RICK_C64 and N in {256, 512, 1024, 2048} only, RICK_EINVAL otherwise;
  * call after rick_plan_set_dtype, which switches it off).  With fusion on, rick_fft_planes runs only the

@@ -21,7 +21,7 @@ _lib = None
 
 EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
-    "rick_plan_sort_layout", "rick_plan_set_fusion",
+    "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
@@ -62,6 +62,7 @@ def lib():
         L.rick_plan_workspace_bytes.argtypes = [vp, ll, C.POINTER(sz), C.POINTER(sz)]
         L.rick_plan_destroy.argtypes = [vp]
         L.rick_plan_set_fusion.argtypes = [vp, i]
+        L.rick_plan_set_kernel.argtypes = [vp, i, dbl]
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
@@ -136,6 +137,14 @@ def rick_plan_set_fusion(plan: int, on: bool) -> bool:
     return bool(on)
 
 
+RICK_KERNEL_GAUSS, RICK_KERNEL_KB = 0, 1
+
+
+def rick_plan_set_kernel(plan: int, kind: int, param: float = 0.0) -> None:
+    """Gridding kernel: RICK_KERNEL_GAUSS (default) or RICK_KERNEL_KB with shape parameter beta = param."""
+    _check(lib().rick_plan_set_kernel(plan, int(kind), float(param)), "rick_plan_set_kernel")
+
+
 def rick_plan_destroy(plan: int) -> None:
     _check(lib().rick_plan_destroy(plan), "rick_plan_destroy")
 
@@ -203,7 +212,8 @@ class Imager:
     points in path order.  Nothing is computed in Python."""
 
     def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
-                 dtype: str = "c64", M_max: int = 0, device="cuda", fused: bool = False):
+                 dtype: str = "c64", M_max: int = 0, device="cuda", fused: bool = False,
+                 kernel: str = "gauss", beta: float = 0.0):
         if not torch.cuda.is_available():
             raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -214,6 +224,10 @@ class Imager:
             self.plan = rick_plan_create(N, Nw, support, sigma, w_min, w_max, dl)
             rick_plan_set_dtype(self.plan, self.dtype)
             self.fused = rick_plan_set_fusion(self.plan, True) if fused else False
+            if kernel == "kb":
+                rick_plan_set_kernel(self.plan, RICK_KERNEL_KB, beta)
+            elif kernel != "gauss":
+                raise RickError(f"unknown gridding kernel {kernel!r}")
         self.M_max = 0
         self.grid = torch.empty((Nw, N, N), dtype=self.cdtype, device=self.device)
         self.image = torch.empty((N, N), dtype=torch.float64, device=self.device)

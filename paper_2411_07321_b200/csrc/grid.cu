@@ -90,6 +90,41 @@ __device__ __forceinline__ void taps(double* t, double d0, const RickGeom& g, co
     }
 }
 
+// Kaiser-Bessel taps [D6-KB]: g(|d|) from the plan's tables over [0, a_t] (built in fp64 on the host).
+// fp32 mesh: linear interpolation between 8192 nodes (error < 4e-8 of the peak); fp64 mesh: cubic Hermite
+// on values and derivatives (error < 1e-14).  d = d0 + a - h lies in (-a_t, a_t].
+template <int S, bool kSigned>
+__device__ __forceinline__ void taps_kb(float* t, float d0, const RickGeom& g) {
+    constexpr int h = (S - 1) / 2;
+    const float inv_h = (float)g.kb_inv_h;
+#pragma unroll
+    for (int a = 0; a < S; ++a) {
+        const float x = fabsf(d0 + (float)(a - h)) * inv_h;
+        int i = (int)x;
+        i = i < g.kb_n ? i : g.kb_n - 1;
+        const float2 e = __ldg(g.kb_lut_f + i);
+        const float v = fmaf(e.y, x - (float)i, e.x);
+        t[a] = (kSigned && (a & 1)) ? -v : v;
+    }
+}
+template <int S, bool kSigned>
+__device__ __forceinline__ void taps_kb(double* t, double d0, const RickGeom& g) {
+    constexpr int h = (S - 1) / 2;
+#pragma unroll
+    for (int a = 0; a < S; ++a) {
+        const double x = fabs(d0 + (double)(a - h)) * g.kb_inv_h;
+        int i = (int)x;
+        i = i < g.kb_n ? i : g.kb_n - 1;
+        const double f = x - (double)i;
+        const double2 e0 = __ldg(g.kb_lut_d + i), e1 = __ldg(g.kb_lut_d + i + 1);
+        // cubic Hermite on [0, 1]: values e0.x, e1.x, scaled slopes e0.y, e1.y
+        const double f2 = f * f, f3 = f2 * f;
+        const double v = (2.0 * f3 - 3.0 * f2 + 1.0) * e0.x + (f3 - 2.0 * f2 + f) * e0.y +
+                         (-2.0 * f3 + 3.0 * f2) * e1.x + (f3 - f2) * e1.y;
+        t[a] = (kSigned && (a & 1)) ? -v : v;
+    }
+}
+
 template <typename real> struct CellOf;
 template <> struct CellOf<float> { typedef float2 type; };
 template <> struct CellOf<double> { typedef double2 type; };
@@ -104,7 +139,7 @@ __device__ __forceinline__ float4 load4(const float* __restrict__ a, long long p
     return r;
 }
 
-template <typename real, int S, int RB>
+template <typename real, int S, int RB, int KIND>
 __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                           const float* __restrict__ u_s, const float* __restrict__ v_s,
                                                           const float* __restrict__ w_s, const float2* __restrict__ vis_s,
@@ -167,12 +202,14 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
                 ci = loc.i0; cj = loc.j0; ck = loc.k;
             }
             real gx[W], gy[S];
-            taps<S, true>(gy, (double)loc.j0 - loc.y, g, tc);
+            if (KIND == RICK_KERNEL_KB) taps_kb<S, true>(gy, (real)((double)loc.j0 - loc.y), g);
+            else taps<S, true>(gy, (double)loc.j0 - loc.y, g, tc);
             bool neg;
             if constexpr (kWin) {
                 // window column c <-> cell iw + c, iw even: sign (-1)^c at compile time; tap index c - o
                 real t[S];
-                taps<S, false>(t, (double)loc.i0 - loc.x, g, tc);
+                if (KIND == RICK_KERNEL_KB) taps_kb<S, false>(t, (real)((double)loc.i0 - loc.x), g);
+                else taps<S, false>(t, (double)loc.i0 - loc.x, g, tc);
                 const bool o = ((loc.i0 - h) & 1) != 0;
 #pragma unroll
                 for (int c = 0; c < W; ++c) {
@@ -182,7 +219,8 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
                 }
                 neg = ((loc.j0 - h) & 1) != 0;            // (-1)^(j0-h): the rest of (-1)^(i+j)
             } else {
-                taps<S, true>(gx, (double)loc.i0 - loc.x, g, tc);
+                if (KIND == RICK_KERNEL_KB) taps_kb<S, true>(gx, (real)((double)loc.i0 - loc.x), g);
+                else taps<S, true>(gx, (double)loc.i0 - loc.x, g, tc);
                 neg = ((loc.i0 + loc.j0) & 1) != 0;       // (-1)^(i0+j0)
             }
             const real ws = neg ? -(real)wgt : (real)wgt;
@@ -229,7 +267,7 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 
-template <int S, int RB, int L, int NBUF>
+template <int S, int RB, int L, int NBUF, int KIND>
 __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                          const uint2* __restrict__ ga, const float2* __restrict__ gb,
                                                          const float2* __restrict__ gc, float2* __restrict__ grid,
@@ -305,8 +343,13 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
                 cij = wij; ck = k;
             }
             float t[S], gx[W], gy[S];
-            taps_f32<S, true>(gy, dy, c2, tc);
-            taps_f32<S, false>(t, dx, c2, tc);
+            if (KIND == RICK_KERNEL_KB) {
+                taps_kb<S, true>(gy, dy, g);
+                taps_kb<S, false>(t, dx, g);
+            } else {
+                taps_f32<S, true>(gy, dy, c2, tc);
+                taps_f32<S, false>(t, dx, c2, tc);
+            }
             const bool o = (((int)(ij & 0xFFFFu) - h) & 1) != 0;     // footprint starts on an odd column
 #pragma unroll
             for (int c = 0; c < W; ++c) {
@@ -359,8 +402,8 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
     }
 }
 
-template <int S, int RB>
-int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
+template <int S, int RB, int KIND>
+int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
     constexpr int L = 16;                                   // records per thread and stage
 #ifndef RICK_GRID_NBUF
 #define RICK_GRID_NBUF 2
@@ -369,7 +412,7 @@ int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
     constexpr int smem = NBUF * 3 * kRunThreads * (L / 2) * 16;   // NBUF buffers of three streams, 48 KB each
     static bool attr_done = false;
     if (!attr_done) {
-        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return RICK_ECUDA;
         attr_done = true;
     }
@@ -385,13 +428,13 @@ int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
     n_stage = n_stage < 2 ? 2 : (n_stage > 16 ? 16 : n_stage);
     const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
-    k_grid_rec<S, RB, L, NBUF><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
+    k_grid_rec<S, RB, L, NBUF, KIND><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
                                                            (float2*)grid, n_stage);
     return RICK_OK;
 }
 
-template <typename real, int S, int RB>
-void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
+template <typename real, int S, int RB, int KIND>
+void launch_runs_k(rick_plan* p, void* grid, cudaStream_t st) {
     typedef typename CellOf<real>::type cell;
     TapConst tc;
     for (int t = 0; t < 8; ++t) {
@@ -404,8 +447,19 @@ void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
     L = L < 32 ? 32 : (L > 256 ? 256 : L);
     const long long per_block = (long long)kRunThreads * L;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
-    k_grid_runs<real, S, RB><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
+    k_grid_runs<real, S, RB, KIND><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
                                                               (const float2*)p->vis_s, p->weight_s, (cell*)grid, (int)L);
+}
+
+template <int S, int RB>
+int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
+    return p->g.kernel == RICK_KERNEL_KB ? launch_rec_k<S, RB, RICK_KERNEL_KB>(p, grid, st)
+                                         : launch_rec_k<S, RB, RICK_KERNEL_GAUSS>(p, grid, st);
+}
+template <typename real, int S, int RB>
+void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {
+    if (p->g.kernel == RICK_KERNEL_KB) launch_runs_k<real, S, RB, RICK_KERNEL_KB>(p, grid, st);
+    else launch_runs_k<real, S, RB, RICK_KERNEL_GAUSS>(p, grid, st);
 }
 
 }  // namespace

@@ -96,6 +96,66 @@ int build_fft(rick_plan* p) {
     return RICK_ECUFFT;
 }
 
+
+// modified Bessel functions by their power series (all terms positive)
+double bessel_i0_series(double x) {
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+double bessel_i1_over_x_series(double x) {     // I1(x) / x = sum_k (x^2/4)^k / (k! (k+1)!) / 2
+    const double q = 0.25 * x * x;
+    double term = 0.5, sum = 0.5;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)(k + 1));
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+
+// D8 / D8-KB: 1 / t[p] on the device.  Gaussian: t[p] = c0 exp(-2 pi^2 sigma^2 nu_p^2),
+// c0 = sigma sqrt(2 pi) erf(a_t / (sigma sqrt 2)).  Kaiser-Bessel: t = 2 a_t sinh(z) / (z I0(beta)),
+// z = sqrt(beta^2 - (2 pi a_t nu)^2) (sin(z') / z' beyond the main lobe).
+int upload_taper(rick_plan* p) {
+    const RickGeom& g = p->g;
+    const int N = g.N;
+    double* inv_t = (double*)malloc(sizeof(double) * (size_t)N);
+    if (!inv_t) return RICK_ENOMEM;
+    const double pi = 3.14159265358979323846;
+    const double a_t = (double)g.h + 0.5;
+    if (g.kernel == RICK_KERNEL_KB) {
+        const double i0b = bessel_i0_series(p->kb_beta);
+        for (int i = 0; i < N; ++i) {
+            const double nu = (double)(i - N / 2) / (double)N;
+            const double y = 2.0 * pi * a_t * nu;
+            const double z2 = p->kb_beta * p->kb_beta - y * y;
+            double sc = 1.0;
+            if (z2 > 1e-24) { const double z = sqrt(z2); sc = sinh(z) / z; }
+            else if (z2 < -1e-24) { const double z = sqrt(-z2); sc = sin(z) / z; }
+            inv_t[i] = i0b / (2.0 * a_t * sc);
+        }
+    } else {
+        const double sigma = g.sigma;
+        const double c0 = sigma * sqrt(2.0 * pi) * erf(a_t / (sigma * sqrt(2.0)));
+        for (int i = 0; i < N; ++i) {
+            const double nu = (double)(i - N / 2) / (double)N;
+            inv_t[i] = 1.0 / (c0 * exp(-2.0 * pi * pi * sigma * sigma * nu * nu));
+        }
+    }
+    cudaError_t e = cudaSuccess;
+    if (!p->inv_taper_dev) e = cudaMalloc((void**)&p->inv_taper_dev, sizeof(double) * (size_t)N);
+    if (e == cudaSuccess) e = cudaMemcpy(p->inv_taper_dev, inv_t, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice);
+    free(inv_t);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RICK_ENOMEM : RICK_ECUDA;
+    return RICK_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -157,25 +217,9 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { delete p; return RICK_ECUDA; }
     p->sm_count = sms > 0 ? sms : 148;
 
-    // D8 1-D taper: t[p] = c0 exp(-2 pi^2 sigma^2 nu_p^2), c0 = sigma sqrt(2 pi) erf((h + 1/2)/(sigma sqrt 2))
-    double* inv_t = (double*)malloc(sizeof(double) * (size_t)N);
-    if (!inv_t) { delete p; return RICK_ENOMEM; }
     {
-        const double pi = 3.14159265358979323846;
-        const double a_t = (double)g.h + 0.5;
-        const double c0 = sigma * sqrt(2.0 * pi) * erf(a_t / (sigma * sqrt(2.0)));
-        for (int i = 0; i < N; ++i) {
-            const double nu = (double)(i - N / 2) / (double)N;
-            inv_t[i] = 1.0 / (c0 * exp(-2.0 * pi * pi * sigma * sigma * nu * nu));
-        }
-    }
-    cudaError_t e = cudaMalloc((void**)&p->inv_taper_dev, sizeof(double) * (size_t)N);
-    if (e == cudaSuccess) e = cudaMemcpy(p->inv_taper_dev, inv_t, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice);
-    free(inv_t);
-    if (e != cudaSuccess) {
-        if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
-        delete p;
-        return e == cudaErrorMemoryAllocation ? RICK_ENOMEM : RICK_ECUDA;
+        const int rc = upload_taper(p);
+        if (rc != RICK_OK) { delete p; return rc; }
     }
     for (int i = 0; i < RICK_T_COUNT; ++i) {
         if (cudaEventCreate(&p->ev_start[i]) != cudaSuccess || cudaEventCreate(&p->ev_stop[i]) != cudaSuccess) {
@@ -192,6 +236,43 @@ int rick_plan_set_dtype(rick_plan* p, int dtype) {
     p->dtype = dtype;
     p->dtype_set = true;
     return build_fft(p);
+}
+
+int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
+    if (!p || (kind != RICK_KERNEL_GAUSS && kind != RICK_KERNEL_KB)) return RICK_EINVAL;
+    if (kind == RICK_KERNEL_KB && !(param > 0.0 && param <= 64.0)) return RICK_EINVAL;
+    RICK_CUDA(cudaDeviceSynchronize());       // the tables may be in use by queued work
+    RickGeom& g = p->g;
+    g.kernel = kind;
+    if (kind == RICK_KERNEL_KB) {
+        p->kb_beta = param;
+        const int nL = 8192;
+        const double a_t = (double)g.h + 0.5, hstep = a_t / nL, i0b = bessel_i0_series(param);
+        float2* lf = (float2*)malloc(sizeof(float2) * (nL + 1));
+        double2* ld = (double2*)malloc(sizeof(double2) * (nL + 1));
+        double* gv = (double*)malloc(sizeof(double) * (nL + 1));
+        if (!lf || !ld || !gv) { free(lf); free(ld); free(gv); return RICK_ENOMEM; }
+        for (int i = 0; i <= nL; ++i) {
+            const double d = i * hstep, r = d / a_t;
+            const double arg = 1.0 - r * r, z = param * sqrt(arg > 0.0 ? arg : 0.0);
+            gv[i] = bessel_i0_series(z) / i0b;
+            // g'(d) = -(beta^2 d / a_t^2) (I1(z) / z) / I0(beta)
+            ld[i] = make_double2(gv[i], hstep * (-(param * param) * d / (a_t * a_t) * bessel_i1_over_x_series(z) / i0b));
+        }
+        for (int i = 0; i <= nL; ++i) lf[i] = make_float2((float)gv[i], i < nL ? (float)(gv[i + 1] - gv[i]) : 0.f);
+        cudaError_t e = cudaSuccess;
+        if (!p->kb_lut_f_dev) e = cudaMalloc(&p->kb_lut_f_dev, sizeof(float2) * (nL + 1));
+        if (e == cudaSuccess && !p->kb_lut_d_dev) e = cudaMalloc(&p->kb_lut_d_dev, sizeof(double2) * (nL + 1));
+        if (e == cudaSuccess) e = cudaMemcpy(p->kb_lut_f_dev, lf, sizeof(float2) * (nL + 1), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p->kb_lut_d_dev, ld, sizeof(double2) * (nL + 1), cudaMemcpyHostToDevice);
+        free(lf); free(ld); free(gv);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RICK_ENOMEM : RICK_ECUDA;
+        g.kb_n = nL;
+        g.kb_inv_h = (double)nL / a_t;
+        g.kb_lut_f = (const float2*)p->kb_lut_f_dev;
+        g.kb_lut_d = (const double2*)p->kb_lut_d_dev;
+    }
+    return upload_taper(p);
 }
 
 int rick_plan_set_fusion(rick_plan* p, int on) {
@@ -231,6 +312,8 @@ int rick_plan_destroy(rick_plan* p) {
     destroy_fft(p);
     if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
     if (p->colfft_tw) cudaFree(p->colfft_tw);
+    if (p->kb_lut_f_dev) cudaFree(p->kb_lut_f_dev);
+    if (p->kb_lut_d_dev) cudaFree(p->kb_lut_d_dev);
     for (int i = 0; i < RICK_T_COUNT; ++i) {
         if (p->ev_start[i]) cudaEventDestroy(p->ev_start[i]);
         if (p->ev_stop[i]) cudaEventDestroy(p->ev_stop[i]);

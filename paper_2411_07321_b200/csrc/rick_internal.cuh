@@ -27,6 +27,12 @@ struct RickGeom {
     int cell_bits;   // cb: in-tile cell bits appended to the tile key in the sort key [D4']
     uint32_t sort_sentinel;  // sort key of a dropped visibility: (n_bins << cb) - 1, a key D5 never keeps
     double tap_c;    // 1 / (2 sigma^2)
+    // Kaiser-Bessel taps (rick_plan_set_kernel): tables over |d| in [0, a_t], kb_n intervals of a_t / kb_n
+    int kernel;                 // RICK_KERNEL_GAUSS / RICK_KERNEL_KB
+    int kb_n;
+    double kb_inv_h;            // kb_n / a_t
+    const float2* kb_lut_f;     // [kb_n + 1] (g_i, g_{i+1} - g_i): linear interpolation, fp32 mesh
+    const double2* kb_lut_d;    // [kb_n + 1] (g_i, (a_t / kb_n) g'_i): cubic Hermite, fp64 mesh
 };
 
 struct rick_plan {
@@ -36,6 +42,8 @@ struct rick_plan {
     // sort layout
     int key_bits, n_pass;
     int digit_bits[RICK_MAX_PASSES], digit_shift[RICK_MAX_PASSES];
+    double kb_beta;
+    void *kb_lut_f_dev, *kb_lut_d_dev;
     // taper: inv_t[p] = 1 / t[p], device double[N]
     double* inv_taper_dev;
     // fused column transform + w-correction (colfft.cu), opt-in

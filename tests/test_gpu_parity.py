@@ -281,3 +281,45 @@ def test_fused_column_transform(name, M, plan):
     im2 = B.Imager(dtype="c128", M_max=16, fused=True, **pa)
     assert not im2.fused
     im2.close()
+
+
+@pytest.mark.parametrize("name,M,plan,dtype,fused", [
+    ("tiny", 100_000, {}, "c128", False),
+    ("10M", 400_000, dict(N=512, Nw=8), "c64", False),
+    ("10M", 400_000, dict(N=512, Nw=8), "c64", True),
+    ("hotspot", 300_001, dict(N=1024, Nw=4), "c64", False),        # support 9
+])
+def test_kaiser_bessel_kernel(name, M, plan, dtype, fused):
+    """rick_plan_set_kernel(RICK_KERNEL_KB): the paper's own gridding kernel [D6-KB, D8-KB]: mesh and
+    image against the oracle, same gates as the Gaussian."""
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    N, beta = pa["N"], 2.34 * pa["support"]
+    oplan = O.Plan(kernel="kb", beta=beta, **pa)
+    hv = vis.numpy()
+    im = B.Imager(dtype=dtype, M_max=M, fused=fused, kernel="kb", beta=beta, **pa)
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
+    im.grid_(True)
+    torch.cuda.synchronize()
+    ii = np.arange(N)
+    cb = np.where((ii[:, None] + ii[None, :]) & 1, -1.0, 1.0)
+    g = im.grid.cpu().numpy().astype(np.complex128) * cb[None]
+    og = O.grid(oplan, *hv)
+    gerr = np.abs(g - og).max() / np.abs(og).max()
+    assert gerr <= (1e-12 if dtype == "c128" else 2e-6), gerr
+    im.fft()
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    img = im.image.cpu().numpy()
+    ref = O.image(oplan, *hv)
+    t = O.taper(N, cfg.support, cfg.sigma, "kb", beta)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    inner = slice(N // 4, 3 * N // 4)
+    peak = np.abs(ref[inner, inner]).max()
+    d = np.abs(img - ref)
+    a, b = d[tw >= 1e-2].max() / peak, (d * tw).max() / peak
+    print(f"KB {name}/{dtype} fused={fused}: grid {gerr:.2e} gateA {a:.2e} gateB {b:.2e}")
+    assert a <= TOL[dtype] and b <= TOL[dtype]
+    # and it is not the Gaussian image (the switch really took effect)
+    gref = O.image(O.Plan(**pa), *hv)
+    assert np.abs(img - gref)[inner, inner].max() > 10 * TOL[dtype] * peak
+    im.close()
