@@ -1,21 +1,26 @@
-// grid.cu -- rick_grid: convolutional gridding, Eq. 3 with the separable truncated Gaussian [D6].
+// grid.cu -- rick_grid: convolutional gridding, Eq. 3, with the separable truncated Gaussian [D6]
+// or the separable Kaiser-Bessel window of the paper's own tests [D6-KB] (rick_plan_set_kernel).
 //
-// Run-accumulating gridder.  rick_bin leaves the kept visibilities sorted by (plane, tile, cell) [D4'],
+// Run-accumulating gridders.  rick_bin leaves the kept visibilities sorted by (plane, tile, cell) [D4'],
 // so visibilities that share a nearest cell (i0, j0, k) -- and therefore the same S x S footprint --
 // are adjacent: 87 % of the "10M" workload sits in runs of >= 8.
 // Each thread walks a range of consecutive sorted visibilities (32 .. 256) and keeps the whole footprint
-// (S*S complex accumulators, or a block of RB rows of it per pass) in registers:
+// (or a block of RB rows of it per pass) in registers:
 //
 //     acc[b][a] += gx[a] * (gy[b] * weight * V)          2 FMAs per cell and visibility
 //
-// and only when the nearest cell changes (or its range ends) adds the footprint to the mesh with
-// vector reductions in L2 (red.global.add.v4.f32, two cells each / red.global.add.f64).  Lanes of a warp hold
-// neighbouring cells, so those reductions fall into the same few sectors.  No shared memory, no
-// shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on sm_100a), and the number
-// of L2 reductions per visibility drops from S*S to S*S / (mean run length clipped to the range).
+// and only when the footprint window changes (or its range ends) adds it to the mesh with reductions in
+// L2.  No shared-memory accumulation: fp32 atomicAdd on shared memory is a CAS loop on sm_100a.
 //
-// The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) costs nothing: (-1)^(a+b) is folded
-// into the taps as compile-time negations and (-1)^(i0+j0) into the sign of the weight.
+//   k_grid_rec  (fp32 mesh)  reads the 24-byte gridder records the gather wrote (cell, plane, fractional
+//               offsets, signed weight * V), staged through shared memory with coalesced cp.async copies;
+//               the footprint columns live in an even-aligned window of S + 1 cells, so every flush is a
+//               16-byte red.global.add.v4.f32 (two cells) and two neighbouring cells share one window.
+//   k_grid_runs (fp64 mesh)  reads the sorted SoA, recomputes the coordinates in fp64 (bit-identical
+//               indices to the key generation), red.global.add.f64 (no vector fp64 reduction exists).
+//
+// The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) costs nothing: the column and row
+// signs are compile-time negations of the taps, the run-constant remainder is the sign of the weight.
 #include "rick_internal.cuh"
 
 namespace {
@@ -405,10 +410,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 template <int S, int RB, int KIND>
 int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
     constexpr int L = 16;                                   // records per thread and stage
-#ifndef RICK_GRID_NBUF
-#define RICK_GRID_NBUF 2
-#endif
-    constexpr int NBUF = RICK_GRID_NBUF;
+    constexpr int NBUF = 2;                                 // double-buffered stages (1 was measured: no gain)
     constexpr int smem = NBUF * 3 * kRunThreads * (L / 2) * 16;   // NBUF buffers of three streams, 48 KB each
     static bool attr_done = false;
     if (!attr_done) {
