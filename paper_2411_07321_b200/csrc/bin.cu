@@ -16,7 +16,7 @@ namespace {
 
 constexpr int kRadix = 1 << RICK_RADIX_BITS_MAX;   // 512 digit values at most
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;
+constexpr int kSortItems = 32;
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kSortWarps = kSortThreads / 32;
 
@@ -169,7 +169,7 @@ struct SortSmem {
 };
 
 template <bool kFirst, int kBits>
-__global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint32_t* __restrict__ key_in,
+__global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __restrict__ key_in,
                                                                const uint32_t* __restrict__ idx_in,
                                                                uint32_t* __restrict__ key_out,
                                                                uint32_t* __restrict__ idx_out, long long M, int shift,
