@@ -21,6 +21,8 @@
 //
 // The checkerboard (-1)^(i+j) of the modulated mesh (rick_b200.h) costs nothing: the column and row
 // signs are compile-time negations of the taps, the run-constant remainder is the sign of the weight.
+#include <string.h>
+
 #include "rick_internal.cuh"
 
 namespace {
@@ -30,6 +32,10 @@ constexpr int kRunThreads = 128;
 struct TapConst {
     double K[8];   // K[t] = exp(-t^2 / (2 sigma^2)), t = 0 .. h
     float Kf[8];   // the same, rounded to fp32
+};
+struct KbPoly {    // Kaiser-Bessel taps as polynomials in 2 delta (plan: kb_poly), fp32 gridder only
+    float c[15][RICK_KB_POLY_TERMS];
+    int ok;        // 0: use the table
 };
 
 __device__ __forceinline__ void red_add_cell(float2* addr, float re, float im) {
@@ -109,6 +115,18 @@ __device__ __forceinline__ void taps_kb(float* t, float d0, const RickGeom& g) {
         i = i < g.kb_n ? i : g.kb_n - 1;
         const float2 e = __ldg(g.kb_lut_f + i);
         const float v = fmaf(e.y, x - (float)i, e.x);
+        t[a] = (kSigned && (a & 1)) ? -v : v;
+    }
+}
+// the same taps from the per-tap polynomials in 2 d0 (no memory access: coefficients are kernel parameters)
+template <int S, bool kSigned>
+__device__ __forceinline__ void taps_kb_poly(float* t, float d0, const KbPoly& kp) {
+    const float x = 2.0f * d0;
+#pragma unroll
+    for (int a = 0; a < S; ++a) {
+        float v = kp.c[a][RICK_KB_POLY_TERMS - 1];
+#pragma unroll
+        for (int k = RICK_KB_POLY_TERMS - 2; k >= 0; --k) v = fmaf(v, x, kp.c[a][k]);
         t[a] = (kSigned && (a & 1)) ? -v : v;
     }
 }
@@ -276,7 +294,7 @@ template <int S, int RB, int L, int NBUF, int KIND>
 __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                          const uint2* __restrict__ ga, const float2* __restrict__ gb,
                                                          const float2* __restrict__ gc, float2* __restrict__ grid,
-                                                         int n_stage) {
+                                                         int n_stage, KbPoly kp) {
     constexpr int h = (S - 1) / 2;
     constexpr int kPasses = (S + RB - 1) / RB;
     constexpr int W = S + 1;                    // even-aligned window, see k_grid_runs
@@ -349,8 +367,13 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             }
             float t[S], gx[W], gy[S];
             if (KIND == RICK_KERNEL_KB) {
-                taps_kb<S, true>(gy, dy, g);
-                taps_kb<S, false>(t, dx, g);
+                if (kp.ok) {
+                    taps_kb_poly<S, true>(gy, dy, kp);
+                    taps_kb_poly<S, false>(t, dx, kp);
+                } else {
+                    taps_kb<S, true>(gy, dy, g);
+                    taps_kb<S, false>(t, dx, g);
+                }
             } else {
                 taps_f32<S, true>(gy, dy, c2, tc);
                 taps_f32<S, false>(t, dx, c2, tc);
@@ -430,8 +453,14 @@ int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
     n_stage = n_stage < 2 ? 2 : (n_stage > 16 ? 16 : n_stage);
     const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
+    KbPoly kp;
+    memset(&kp, 0, sizeof(kp));
+    if (KIND == RICK_KERNEL_KB && p->kb_poly_ok) {
+        memcpy(kp.c, p->kb_poly, sizeof(kp.c));
+        kp.ok = 1;
+    }
     k_grid_rec<S, RB, L, NBUF, KIND><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
-                                                           (float2*)grid, n_stage);
+                                                           (float2*)grid, n_stage, kp);
     return RICK_OK;
 }
 

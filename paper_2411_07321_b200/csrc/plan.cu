@@ -156,6 +156,47 @@ int upload_taper(rick_plan* p) {
     return RICK_OK;
 }
 
+
+// Degree-(T-1) interpolation polynomials (in t = 2 delta) of the Kaiser-Bessel taps g(delta + a - h) at the T
+// Chebyshev nodes of [-1, 1]; returns the largest error of the fp32-rounded polynomials over a fine sample.
+double fit_kb_polynomials(rick_plan* p) {
+    const int T = RICK_KB_POLY_TERMS, S = p->g.S, h = p->g.h;
+    const double a_t = (double)h + 0.5, beta = p->kb_beta, i0b = bessel_i0_series(beta), pi = 3.14159265358979323846;
+    auto win = [&](double d) {
+        const double r = d / a_t, arg = 1.0 - r * r;
+        return bessel_i0_series(beta * sqrt(arg > 0.0 ? arg : 0.0)) / i0b;
+    };
+    double worst = 0.0;
+    for (int a = 0; a < S; ++a) {
+        long double A[RICK_KB_POLY_TERMS][RICK_KB_POLY_TERMS + 1];
+        for (int r = 0; r < T; ++r) {
+            const double t = cos(pi * (2.0 * r + 1.0) / (2.0 * T));
+            long double pw = 1.0L;
+            for (int c = 0; c < T; ++c) { A[r][c] = pw; pw *= (long double)t; }
+            A[r][T] = (long double)win(0.5 * t + (double)(a - h));
+        }
+        for (int c = 0; c < T; ++c) {                      // Gauss-Jordan with partial pivoting
+            int piv = c;
+            for (int r = c + 1; r < T; ++r) if (fabsl(A[r][c]) > fabsl(A[piv][c])) piv = r;
+            for (int k = 0; k <= T; ++k) { const long double tmp = A[c][k]; A[c][k] = A[piv][k]; A[piv][k] = tmp; }
+            for (int r = 0; r < T; ++r) {
+                if (r == c) continue;
+                const long double f = A[r][c] / A[c][c];
+                for (int k = c; k <= T; ++k) A[r][k] -= f * A[c][k];
+            }
+        }
+        for (int c = 0; c < T; ++c) p->kb_poly[a][c] = (float)(A[c][T] / A[c][c]);
+        for (int i = 0; i <= 400; ++i) {
+            const double t = -1.0 + i / 200.0;
+            double v = 0.0;
+            for (int c = T - 1; c >= 0; --c) v = v * t + (double)p->kb_poly[a][c];
+            const double e = fabs(v - win(0.5 * t + (double)(a - h)));
+            if (e > worst) worst = e;
+        }
+    }
+    return worst;
+}
+
 }  // namespace
 
 extern "C" {
@@ -271,6 +312,7 @@ int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
         g.kb_inv_h = (double)nL / a_t;
         g.kb_lut_f = (const float2*)p->kb_lut_f_dev;
         g.kb_lut_d = (const double2*)p->kb_lut_d_dev;
+        p->kb_poly_ok = fit_kb_polynomials(p) <= 5e-8;
     }
     return upload_taper(p);
 }

@@ -10,6 +10,7 @@
 
 #define RICK_TILE 32          // uv tile edge of the sort key (BASELINE.json north_star (2))
 #define RICK_MAX_PASSES 4
+#define RICK_KB_POLY_TERMS 10
 #define RICK_GREC_PAD 4096    // gridder records are allocated in whole chunks of this many (one CTA's share)
 #define RICK_RADIX_BITS_MAX 9
 
@@ -44,6 +45,11 @@ struct rick_plan {
     int digit_bits[RICK_MAX_PASSES], digit_shift[RICK_MAX_PASSES];
     double kb_beta;
     void *kb_lut_f_dev, *kb_lut_d_dev;
+    // per-tap polynomials of the Kaiser-Bessel window for the fp32 gridder: tap a of a visibility with
+    // fractional offset delta in [-1/2, 1/2] is sum_k kb_poly[a][k] (2 delta)^k (fitted in fp64 at
+    // rick_plan_set_kernel, used when the fit is good to 5e-8 of the peak: kb_poly_ok)
+    float kb_poly[15][RICK_KB_POLY_TERMS];
+    bool kb_poly_ok;
     // taper: inv_t[p] = 1 / t[p], device double[N]
     double* inv_taper_dev;
     // fused column transform + w-correction (colfft.cu), opt-in
