@@ -269,8 +269,10 @@ def main():
     _, n_pass, _ = B.rick_plan_sort_layout(im.plan)
     alg = {   # algorithmic bytes per launch
         "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
-        "sort": (12 + 16 * (n_pass - 1)) * M,        # first pass 4 r + 8 w, later passes 8 r + 8 w
-        "gather": (4 + 32 + 24) * n_kept,            # index + record in, sorted SoA out
+        # sort: first pass 4 r + 8 w, middle passes 8 r + 8 w, last pass 8 r and, fused into it, the gather
+        # (one 32-B record in, sorted SoA 24 B + gridder records 24 B out per kept visibility)
+        "sort": ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept,
+        "gather": 0,                                 # rides in the last sort pass (rick_bin without perm_out)
         "zero": mesh_bytes,
         "grid": 24 * n_kept,
         "fft": (2 if im.fused else 4) * mesh_bytes,      # fused: row transforms only (one read + write)
@@ -278,6 +280,8 @@ def main():
     }
     stages = {}
     for k, b in alg.items():
+        if k == "gather":
+            continue
         t = stage_ms[k]
         stages[k] = {"ms": round(t, 4), "alg_bytes": b, "gbs": (b / (t * 1e-3) / 1e9) if t > 0 else None,
                      "frac": (b / (t * 1e-3) / 1e9 / peak) if t > 0 else None}
@@ -290,7 +294,7 @@ def main():
     # are per launch (sort: n_pass launches of k_onesweep, the average pass)
     kernels = {"grid": ("k_grid_rec" if cfg.dtype == "c64" else "k_grid_runs", 1),
                "wcorrect": ("k_colfft_wcorrect" if im.fused else "k_wcorrect", 1), "keygen": ("k_keygen", 1),
-               "sort": ("k_onesweep", n_pass), "gather": ("k_gather", 1)}
+               "sort": ("k_onesweep", n_pass)}
     dom = max(kernels, key=lambda k: stage_ms[k])
     kname, n_launch = kernels[dom]
     launch_ms = stage_ms[dom] / n_launch

@@ -158,6 +158,34 @@ __device__ __forceinline__ void st_status(unsigned long long* p, unsigned long l
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// Outputs of the gather: sorted SoA copies and gridder records (rick_internal.cuh) of the kept visibilities.
+struct GatherOut {
+    RickGeom g;
+    const float4* rec;
+    float *u_s, *v_s, *w_s;
+    float2* vis_s;
+    float* wt_s;
+    uint2* ga;
+    float2 *gb, *gc;
+};
+
+// input visibility `src` goes to sorted position `pos`: one 32-byte record read, SoA + record writes; the
+// fp64 coordinate arithmetic is repeated here because the kernel waits on memory anyway
+__device__ __forceinline__ void gather_one(const GatherOut& o, size_t src, size_t pos) {
+    const float4 a = __ldg(o.rec + 2 * src);
+    const float4 b = __ldg(o.rec + 2 * src + 1);
+    o.u_s[pos] = a.x;
+    o.v_s[pos] = a.y;
+    o.w_s[pos] = a.z;
+    o.vis_s[pos] = make_float2(a.w, b.x);
+    o.wt_s[pos] = b.y;
+    const RickLoc r = rick_locate(o.g, a.x, a.y, a.z);
+    const float ws = ((r.j0 - o.g.h) & 1) ? -b.y : b.y;       // (-1)^(j0-h): checkerboard factor of the fp32 gridder
+    o.ga[pos] = make_uint2((uint32_t)r.i0 | ((uint32_t)r.j0 << 16), (uint32_t)r.k);
+    o.gb[pos] = make_float2((float)((double)r.i0 - r.x), (float)((double)r.j0 - r.y));
+    o.gc[pos] = make_float2(ws * a.w, ws * b.x);
+}
+
 struct SortSmem {
     uint32_t warp_cnt[kSortWarps][kRadix];   // per-warp digit counts -> exclusive offsets over warps
     uint32_t tile_excl[kRadix];              // first slot of each digit in the exchanged tile
@@ -168,14 +196,18 @@ struct SortSmem {
     uint32_t tile;
 };
 
-template <bool kFirst, int kBits>
+// kGather: this is the last pass and nobody asked for the sorted (key, index) arrays: instead of writing them,
+// the tile gathers its visibilities straight to their final positions (the gather's random reads hide
+// under the pass's arithmetic, and 12 bytes per visibility of key/index traffic disappear).
+template <bool kFirst, int kBits, bool kGather>
 __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __restrict__ key_in,
                                                                const uint32_t* __restrict__ idx_in,
                                                                uint32_t* __restrict__ key_out,
                                                                uint32_t* __restrict__ idx_out, long long M, int shift,
                                                                const uint32_t* __restrict__ digit_base,
                                                                unsigned long long* __restrict__ status,
-                                                               uint32_t* __restrict__ ticket, uint32_t epoch) {
+                                                               uint32_t* __restrict__ ticket, uint32_t epoch,
+                                                               GatherOut go) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -325,8 +357,12 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
         const uint32_t kk = sm.xkey[i];
         const uint32_t d = (kk >> shift) & mask;
         const uint32_t pos = sm.glob[d] + (uint32_t)i;
-        key_out[pos] = kk;
-        idx_out[pos] = sm.xidx[i];
+        if (kGather) {
+            if (kk != go.g.sort_sentinel) gather_one(go, (size_t)sm.xidx[i], (size_t)pos);   // kept: pos < n_kept
+        } else {
+            key_out[pos] = kk;
+            idx_out[pos] = sm.xidx[i];
+        }
     }
 }
 
@@ -336,29 +372,12 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
 // and weight * V with the run-constant checkerboard factor (-1)^(j0-h) of the fp32 gridder folded in.
 // The kernel waits on memory, so the fp64 coordinate arithmetic is free here.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_gather(RickGeom g, const long long* __restrict__ n_kept,
-                                                const uint32_t* __restrict__ idx, const float4* __restrict__ rec,
-                                                float* __restrict__ u_s, float* __restrict__ v_s,
-                                                float* __restrict__ w_s, float2* __restrict__ vis_s,
-                                                float* __restrict__ wt_s, uint2* __restrict__ ga,
-                                                float2* __restrict__ gb, float2* __restrict__ gc) {
+__global__ void __launch_bounds__(256) k_gather(GatherOut o, const long long* __restrict__ n_kept,
+                                                const uint32_t* __restrict__ idx) {
     const long long n = *n_kept;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const size_t src = (size_t)__ldg(idx + i);
-        const float4 a = __ldg(rec + 2 * src);
-        const float4 b = __ldg(rec + 2 * src + 1);
-        u_s[i] = a.x;
-        v_s[i] = a.y;
-        w_s[i] = a.z;
-        vis_s[i] = make_float2(a.w, b.x);
-        wt_s[i] = b.y;
-        const RickLoc r = rick_locate(g, a.x, a.y, a.z);
-        const float ws = ((r.j0 - g.h) & 1) ? -b.y : b.y;
-        ga[i] = make_uint2((uint32_t)r.i0 | ((uint32_t)r.j0 << 16), (uint32_t)r.k);
-        gb[i] = make_float2((float)((double)r.i0 - r.x), (float)((double)r.j0 - r.y));
-        gc[i] = make_float2(ws * a.w, ws * b.x);
-    }
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        gather_one(o, (size_t)__ldg(idx + i), (size_t)i);
 }
 
 // bin_start[b] = number of sorted tile keys < b, b = 0 .. n_bins + 1
@@ -383,10 +402,14 @@ size_t rick_bin_workspace_bytes(const rick_plan* p, long long M) {
 int rick_bin_init() {
     const int bytes = (int)sizeof(SortSmem);
     const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
-    if (cudaFuncSetAttribute(k_onesweep<true, 8>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 9>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 8>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 9>, a, bytes) != cudaSuccess)
+    if (cudaFuncSetAttribute(k_onesweep<true, 8, false>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, false>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, false>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, false>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 8, true>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, true>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, true>, a, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, true>, a, bytes) != cudaSuccess)
         return RICK_ECUDA;
     return RICK_OK;
 }
@@ -431,38 +454,51 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         const unsigned n_tiles = (unsigned)((M + kSortTile - 1) / kSortTile);
         uint32_t *kin = ws.key_a, *iin = ws.idx_a, *kout = ws.key_b, *iout = ws.idx_b;
         (void)iout;
+        // the gather rides in the last pass unless the caller wants the sorted (key, index) arrays
+        const bool fuse_gather = !perm_out && !bin_start_out;
+        GatherOut go;
+        go.g = g; go.rec = ws.rec;
+        go.u_s = u_s; go.v_s = v_s; go.w_s = w_s; go.vis_s = vis_s; go.wt_s = weight_s;
+        go.ga = nullptr; go.gb = ws.grec_b; go.gc = ws.grec_c;
         for (int pass = 0; pass < p->n_pass; ++pass) {
             const bool first = (pass == 0);
             const bool nine = (lay.bits[pass] == 9);
-            auto kern = first ? (nine ? k_onesweep<true, 9> : k_onesweep<true, 8>)
-                              : (nine ? k_onesweep<false, 9> : k_onesweep<false, 8>);
+            const bool gath = fuse_gather && pass == p->n_pass - 1;
+            if (gath) go.ga = (uint2*)kout;       // this pass writes no (key, index): the pair holds records a[]
+            auto kern = gath ? (first ? (nine ? k_onesweep<true, 9, true> : k_onesweep<true, 8, true>)
+                                      : (nine ? k_onesweep<false, 9, true> : k_onesweep<false, 8, true>))
+                             : (first ? (nine ? k_onesweep<true, 9, false> : k_onesweep<true, 8, false>)
+                                      : (nine ? k_onesweep<false, 9, false> : k_onesweep<false, 8, false>));
             kern<<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
                                                                  ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
-                                                                 (uint32_t)(pass + 1));
+                                                                 (uint32_t)(pass + 1), go);
             RICK_LAUNCH_CHECK();
             p->launches++;
+            if (gath) break;
             uint32_t* t;
             t = kin; kin = kout; kout = t;
             t = iin; iin = iout; iout = t;
         }
         rick_stage_end(p, RICK_T_SORT, st);
-        // sorted (key, index) now live in kin / iin
-        if (perm_out) {
-            RICK_CUDA(cudaMemcpyAsync(perm_out, iin, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
-        }
-        if (bin_start_out) {
-            const long long want = (M + 1 + 255) / 256;
-            const long long cap = (long long)p->sm_count * 16;
-            k_bin_start<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, M, kin, bin_start_out);
-            RICK_LAUNCH_CHECK();
-            p->launches++;
-        }
         rick_stage_begin(p, RICK_T_GATHER, st);
-        {
+        if (fuse_gather) {
+            p->grec_a = (const uint2*)kout;
+        } else {
+            // sorted (key, index) now live in kin / iin
+            if (perm_out) {
+                RICK_CUDA(cudaMemcpyAsync(perm_out, iin, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
+            }
+            if (bin_start_out) {
+                const long long want = (M + 1 + 255) / 256;
+                const long long cap = (long long)p->sm_count * 16;
+                k_bin_start<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, M, kin, bin_start_out);
+                RICK_LAUNCH_CHECK();
+                p->launches++;
+            }
             const long long want = (M + 255) / 256;
             const long long cap = (long long)p->sm_count * 32;
-            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, n_kept_dev, iin, ws.rec, u_s, v_s, w_s, vis_s,
-                                                                     weight_s, (uint2*)kout, ws.grec_b, ws.grec_c);
+            go.ga = (uint2*)kout;
+            k_gather<<<(int)(want > cap ? cap : want), 256, 0, st>>>(go, n_kept_dev, iin);
             RICK_LAUNCH_CHECK();
             p->launches++;
             p->grec_a = (const uint2*)kout;
