@@ -193,6 +193,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fusion", action="store_true", help="2-D cuFFT + separate w-correction kernel")
+    ap.add_argument("--fusion", type=int, default=2, choices=[1, 2],
+                    help="rick_plan_set_fusion mode where the plan supports it: 1 fused column transform, 2 + row occupancy")
     ap.add_argument("--kernel", default="gauss", choices=["gauss", "kb"],
                     help="gridding kernel: the Gaussian of BASELINE.json (default) or the paper's Kaiser-Bessel (beta = 2.34 S)")
     ap.add_argument("--e2e-steps", type=int, default=5)
@@ -223,7 +225,7 @@ def main():
     vis = W.generate(cfg, device=dev)
     pa = W.plan_args(cfg, vis)
     M = vis.M
-    im = B.Imager(dtype=cfg.dtype, M_max=M, fused=not args.no_fusion, kernel=args.kernel, beta=2.34 * cfg.support, **pa)
+    im = B.Imager(dtype=cfg.dtype, M_max=M, fused=0 if args.no_fusion else args.fusion, kernel=args.kernel, beta=2.34 * cfg.support, **pa)
     cell = 16 if cfg.dtype == "c128" else 8
     mesh_bytes = cfg.Nw * cfg.N * cfg.N * cell
 
@@ -334,7 +336,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
         "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
-                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype, "fused_column_transform": bool(im.fused),
+                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype, "fusion_mode": int(im.fused),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs (240 MB) and mesh (1.07 GB) exceed the 126 MB L2; no explicit flush"
                    if args.config == "10M" else "inputs and mesh exceed L2; no explicit flush"},

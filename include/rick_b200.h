@@ -90,10 +90,14 @@ int rick_plan_set_dtype(rick_plan* plan, int dtype);
 int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
 
 /* Fused column transform (optional; RICK_C64 and N in {256, 512, 1024, 2048} only, RICK_EINVAL otherwise;
- * call after rick_plan_set_dtype, which switches it off).  With fusion on, rick_fft_planes runs only the
- * row transforms of D7 (the mesh then holds row-transformed planes), and rick_wcorrect_accumulate
- * performs the column transforms itself, fused with the phase screen, the plane sum and the taper
- * division, in one read of the mesh [D7, D8].  The image is the same within fp32 round-off. */
+ * call after rick_plan_set_dtype, which switches it off, and before rick_bin).
+ * on = 1: rick_fft_planes runs only the row transforms of D7 (the mesh then holds row-transformed planes),
+ * and rick_wcorrect_accumulate performs the column transforms itself, fused with the phase screen, the plane
+ * sum and the taper division, in one read of the mesh [D7, D8]; the image is the same within fp32 round-off.
+ * on = 2: in addition the library tracks which mesh rows (plane, j) some footprint touches: rick_grid clears
+ * only touched rows that are not defined yet (instead of the whole mesh) and the fused kernel reads only
+ * defined rows; mesh rows no footprint touches then hold UNDEFINED data (only the image is an output).
+ * on = 0: off. */
 int rick_plan_set_fusion(rick_plan* plan, int on);
 
 /* Sizes of the two caller-provided scratch buffers: `bin_bytes` for rick_bin with up to M

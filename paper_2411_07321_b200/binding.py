@@ -128,13 +128,15 @@ def rick_plan_sort_layout(plan: int):
     return int(a.value), int(b.value), int(c.value)
 
 
-def rick_plan_set_fusion(plan: int, on: bool) -> bool:
-    """Switch the fused column-transform + w-correction path on/off; False when the plan does not support it."""
-    rc = lib().rick_plan_set_fusion(plan, 1 if on else 0)
+def rick_plan_set_fusion(plan: int, on: int) -> int:
+    """Fused column transform: 0 off, 1 on, 2 on + row-occupancy tracking (rick_b200.h).  Returns the mode in
+    force: 0 when the plan does not support fusion."""
+    on = int(on)
+    rc = lib().rick_plan_set_fusion(plan, on)
     if rc == -1 and on:      # RICK_EINVAL: dtype / N not supported by the fused kernel
-        return False
+        return 0
     _check(rc, "rick_plan_set_fusion")
-    return bool(on)
+    return on
 
 
 RICK_KERNEL_GAUSS, RICK_KERNEL_KB = 0, 1
@@ -212,7 +214,7 @@ class Imager:
     points in path order.  Nothing is computed in Python."""
 
     def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
-                 dtype: str = "c64", M_max: int = 0, device="cuda", fused: bool = False,
+                 dtype: str = "c64", M_max: int = 0, device="cuda", fused: int = 0,
                  kernel: str = "gauss", beta: float = 0.0):
         if not torch.cuda.is_available():
             raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
@@ -223,7 +225,7 @@ class Imager:
         with torch.cuda.device(self.device):
             self.plan = rick_plan_create(N, Nw, support, sigma, w_min, w_max, dl)
             rick_plan_set_dtype(self.plan, self.dtype)
-            self.fused = rick_plan_set_fusion(self.plan, True) if fused else False
+            self.fused = rick_plan_set_fusion(self.plan, int(fused)) if fused else 0
             if kernel == "kb":
                 rick_plan_set_kernel(self.plan, RICK_KERNEL_KB, beta)
             elif kernel != "gauss":

@@ -505,6 +505,11 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         }
         rick_stage_end(p, RICK_T_GATHER, st);
     }
+    if (p->fused == 2) {
+        p->n_kept_dev = n_kept_dev;
+        const int rc = rick_rows_mark(p, M, st);
+        if (rc != RICK_OK) return rc;
+    }
     p->M = M;
     p->u_s = u_s; p->v_s = v_s; p->w_s = w_s; p->vis_s = vis_s; p->weight_s = weight_s;
     p->n_kept_dev = n_kept_dev;

@@ -152,7 +152,8 @@ template <int LOG2N>
 __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const float2* __restrict__ planes,
                                                            const float2* __restrict__ tw_g,
                                                            const double* __restrict__ inv_t,
-                                                           double* __restrict__ image, int accumulate) {
+                                                           double* __restrict__ image, int accumulate,
+                                                           const uint32_t* __restrict__ occ, int perm) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 1 << LOG2N;
     constexpr int R3 = N >> 8;                        // radices 16 x 16 x R3
@@ -178,10 +179,14 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 
     auto issue = [&](int k, float2* buf) {
         const float2* src = planes + (size_t)k * N * N + p0;
-        // row j: kC float2 = 32 B = two 16-byte pieces
+        // row j: kC float2 = 32 B = two 16-byte pieces.  Fusion mode 2 (occ != NULL): rows no footprint
+        // touched hold undefined data and are not read -- their slots are zero-filled instead.
         for (int q = tid; q < N * 2; q += kT) {
             const int j = q >> 1, half = q & 1;
-            cp_async16(buf + padded(j * kC + half * 2), src + (size_t)j * N + half * 2);
+            float2* dst = buf + padded(j * kC + half * 2);
+            const bool live = !occ || ((__ldg(occ + ((k * N + j) >> 5)) >> (j & 31)) & 1u);
+            if (live) cp_async16(dst, src + (size_t)j * N + half * 2);
+            else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -197,7 +202,9 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 #pragma unroll
     for (int e = 0; e < per_thread; ++e) {
         const int idx = owned_slot(e);
-        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
+        // perm: the rows were transformed by k_rowfft, which leaves column p at stored position s with
+        // p = slot_to_freq(s) (digit-reversed, never un-permuted)
+        const int q = slot_to_freq(idx / kC, N), sc = p0 + (idx % kC), p = perm ? slot_to_freq(sc, N) : sc;
         const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
         const double r2 = l * l + m * m;
         nm1r[e] = -r2 / (1.0 + sqrt(1.0 - r2));
@@ -245,7 +252,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 #pragma unroll
     for (int e = 0; e < per_thread; ++e) {
         const int idx = owned_slot(e);
-        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
+        const int q = slot_to_freq(idx / kC, N), sc = p0 + (idx % kC), p = perm ? slot_to_freq(sc, N) : sc;
         const double sg = ((p + q) & 1) ? -1.0 : 1.0;
         double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
         const size_t o = (size_t)q * N + p;
@@ -255,6 +262,85 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
             if (accumulate) out += image[o];
             image[o] = out;
         }
+    }
+}
+
+// Row transforms of the listed mesh rows only (fusion mode 2), in place: four rows per step go through the
+// same shared-memory layout and DIF passes as four columns do in k_colfft_wcorrect; the result is written
+// back in the transform's own digit-reversed order (stored position s holds frequency slot_to_freq(s)):
+// the column kernel reads 4 stored-adjacent columns at a time and does not care which they are.
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+template <int LOG2N>
+__global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, const float2* __restrict__ tw_g,
+                                                  const uint32_t* __restrict__ list, const uint32_t* __restrict__ n_rows) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int N = 1 << LOG2N;
+    constexpr int R3 = N >> 8;
+    constexpr int n_slots = N * kC;
+    constexpr int buf_elems = n_slots + ((n_slots >> kPadShift) << 2);
+    float2* buf0 = reinterpret_cast<float2*>(smem_raw);
+    float2* buf1 = buf0 + buf_elems;
+    float2* tw = buf1 + buf_elems;
+    const int tid = threadIdx.x;
+    const int n = (int)*n_rows;
+    const int n_groups = (n + kC - 1) / kC;
+
+    auto issue = [&](int grp, float2* buf) {
+        // slot (i, c) <- element i of row list[4 grp + c]; consecutive threads take consecutive i (coalesced)
+        for (int q = tid; q < N * kC; q += kT) {
+            const int c = q >> LOG2N, i = q & (N - 1);
+            const int r = grp * kC + c;
+            if (r < n) cp_async8(buf + padded(i * kC + c), planes + (size_t)list[r] * N + i);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    int grp = blockIdx.x;
+    if (grp >= n_groups) return;
+    issue(grp, buf0);
+    for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
+    int par = 0;
+    for (; grp < n_groups; grp += gridDim.x, par ^= 1) {
+        float2* buf = par ? buf1 : buf0;
+        const int next = grp + gridDim.x;
+        if (next < n_groups) issue(next, par ? buf0 : buf1);
+        else asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncthreads();
+        dif_pass<LOG2N, 16, LOG2N>(buf, tw, tid);
+        __syncthreads();
+        dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid);
+        __syncthreads();
+        if (R3 > 1) {
+            // last pass straight to global memory: butterfly (B, c) yields stored positions B R3 .. B R3 + R3 - 1 of row c
+#pragma unroll
+            for (int bi = 0; bi < n_slots / kT / R3; ++bi) {
+                const int w = bi * kT + tid;
+                const int B = w / kC, c = w % kC;
+                const int pb = padded(B * (R3 * kC) + c);
+                float2 v[R3];
+#pragma unroll
+                for (int t = 0; t < R3; ++t) v[t] = buf[pb + t * kC];
+                dft<R3>(v);
+                const int r = grp * kC + c;
+                if (r < n) {
+                    float4* dst = reinterpret_cast<float4*>(planes + (size_t)list[r] * N + B * R3);
+#pragma unroll
+                    for (int u = 0; u < R3; u += 2) dst[u >> 1] = make_float4(v[u].x, v[u].y, v[u + 1].x, v[u + 1].y);
+                }
+            }
+        } else {
+            for (int q = tid; q < N * kC; q += kT) {
+                const int c = q >> LOG2N, i = q & (N - 1);
+                const int r = grp * kC + c;
+                if (r < n) planes[(size_t)list[r] * N + i] = buf[padded(i * kC + c)];
+            }
+        }
+        __syncthreads();                              // buf is free for the group after next
     }
 }
 
@@ -310,11 +396,41 @@ int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int
     const float2* planes = (const float2*)grid;
     const float2* tw = (const float2*)p->colfft_tw;
     const int acc = zero_first ? 0 : 1;
+    const uint32_t* occ = p->fused == 2 ? p->occ_mesh_dev : nullptr;
+    const int perm = p->fused == 2 ? 1 : 0;
     switch (N) {
-        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
-        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
-        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
-        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc); break;
+        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
+        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
+        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
+        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
+        default: return RICK_EINVAL;
+    }
+    RICK_LAUNCH_CHECK();
+    p->launches++;
+    return RICK_OK;
+}
+
+int rick_rowfft_impl(rick_plan* p, void* grid, cudaStream_t st) {
+    const int N = p->g.N;
+    const size_t smem = colfft_smem_bytes(N);
+    static bool attr_done = false;
+    if (!attr_done) {
+        const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
+        if (cudaFuncSetAttribute(k_rowfft<8>, a, (int)colfft_smem_bytes(256)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<9>, a, (int)colfft_smem_bytes(512)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<10>, a, (int)colfft_smem_bytes(1024)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<11>, a, (int)colfft_smem_bytes(2048)) != cudaSuccess)
+            return RICK_ECUDA;
+        attr_done = true;
+    }
+    float2* planes = (float2*)grid;
+    const float2* tw = (const float2*)p->colfft_tw;
+    const unsigned blocks = (unsigned)p->sm_count;      // one CTA per SM, each walks its share of row groups
+    switch (N) {
+        case 256: k_rowfft<8><<<blocks, kT, smem, st>>>(planes, tw, p->row_list_dev, p->n_rows_dev); break;
+        case 512: k_rowfft<9><<<blocks, kT, smem, st>>>(planes, tw, p->row_list_dev, p->n_rows_dev); break;
+        case 1024: k_rowfft<10><<<blocks, kT, smem, st>>>(planes, tw, p->row_list_dev, p->n_rows_dev); break;
+        case 2048: k_rowfft<11><<<blocks, kT, smem, st>>>(planes, tw, p->row_list_dev, p->n_rows_dev); break;
         default: return RICK_EINVAL;
     }
     RICK_LAUNCH_CHECK();

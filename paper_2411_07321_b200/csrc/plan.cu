@@ -43,7 +43,7 @@ void destroy_fft(rick_plan* p) {
         p->fft_rows_ready = false;
     }
     p->fft_rows_work_bytes = 0;
-    p->fused = false;
+    p->fused = 0;
 }
 
 // batched 1-D inverse transforms of all Nw * N rows, in place (the row half of D7)
@@ -319,7 +319,8 @@ int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
 
 int rick_plan_set_fusion(rick_plan* p, int on) {
     if (!p) return RICK_EINVAL;
-    if (!on) { p->fused = false; return RICK_OK; }
+    if (on < 0 || on > 2) return RICK_EINVAL;
+    if (!on) { p->fused = 0; return RICK_OK; }
     if (!p->dtype_set) return RICK_ESTATE;
     if (!rick_colfft_supported(p)) return RICK_EINVAL;
     if (!p->fft_rows_ready) {
@@ -327,7 +328,17 @@ int rick_plan_set_fusion(rick_plan* p, int on) {
         if (rc != RICK_OK) return rc;
         if ((rc = rick_colfft_init(p)) != RICK_OK) return rc;
     }
-    p->fused = true;
+    if (on == 2 && !p->occ_cur_dev) {
+        const size_t words = (size_t)p->g.Nw * p->g.N / 32, rows = (size_t)p->g.Nw * p->g.N;
+        if (cudaMalloc((void**)&p->occ_cur_dev, 4 * words) != cudaSuccess ||
+            cudaMalloc((void**)&p->occ_mesh_dev, 4 * words) != cudaSuccess ||
+            cudaMalloc((void**)&p->row_list_dev, 4 * rows) != cudaSuccess ||
+            cudaMalloc((void**)&p->n_rows_dev, 4) != cudaSuccess)
+            return RICK_ENOMEM;
+        RICK_CUDA(cudaMemset(p->occ_cur_dev, 0, 4 * words));
+        RICK_CUDA(cudaMemset(p->occ_mesh_dev, 0, 4 * words));
+    }
+    p->fused = on;
     return RICK_OK;
 }
 
@@ -354,6 +365,10 @@ int rick_plan_destroy(rick_plan* p) {
     destroy_fft(p);
     if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
     if (p->colfft_tw) cudaFree(p->colfft_tw);
+    if (p->occ_cur_dev) cudaFree(p->occ_cur_dev);
+    if (p->occ_mesh_dev) cudaFree(p->occ_mesh_dev);
+    if (p->row_list_dev) cudaFree(p->row_list_dev);
+    if (p->n_rows_dev) cudaFree(p->n_rows_dev);
     if (p->kb_lut_f_dev) cudaFree(p->kb_lut_f_dev);
     if (p->kb_lut_d_dev) cudaFree(p->kb_lut_d_dev);
     for (int i = 0; i < RICK_T_COUNT; ++i) {
@@ -382,7 +397,11 @@ int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
     if (!p || !grid) return RICK_EINVAL;
     if (!p->bound) return RICK_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (zero_first) {
+    if (p->fused == 2) {          // clear only the rows the bound visibilities touch and that are not defined yet
+        StageTimer tz(p, RICK_T_ZERO, st);
+        const int rc = rick_rows_clear(p, grid, zero_first, st);
+        if (rc != RICK_OK) return rc;
+    } else if (zero_first) {
         StageTimer tz(p, RICK_T_ZERO, st);
         const size_t cell = (p->dtype == RICK_C128) ? 16 : 8;
         RICK_CUDA(cudaMemsetAsync(grid, 0, cell * (size_t)p->g.Nw * (size_t)p->g.N * (size_t)p->g.N, st));
@@ -396,6 +415,12 @@ int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_by
     if (!p->fft_ready) return RICK_ESTATE;
     if (p->fft_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_work_bytes)) return RICK_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
+    if (p->fused == 2) {   // row transforms of the defined rows only, by the library's own kernel (colfft.cu)
+        StageTimer tm(p, RICK_T_FFT, st);
+        int rc = rick_rows_list_all(p, st);
+        if (rc == RICK_OK) rc = rick_rowfft_impl(p, grid, st);
+        return rc;
+    }
     if (p->fused) {   // rows only; rick_wcorrect_accumulate finishes the transform (colfft.cu)
         if (p->fft_rows_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_rows_work_bytes)) return RICK_ENOMEM;
         if (cufftSetStream(p->fft_rows, st) != CUFFT_SUCCESS) return RICK_ECUFFT;

@@ -53,7 +53,13 @@ struct rick_plan {
     // taper: inv_t[p] = 1 / t[p], device double[N]
     double* inv_taper_dev;
     // fused column transform + w-correction (colfft.cu), opt-in
-    bool fused;              // rick_plan_set_fusion: rick_fft_planes does rows only, K6 finishes
+    int fused;               // rick_plan_set_fusion: 0 off; 1: rick_fft_planes does rows only, K6 finishes;
+                             // 2: in addition only the mesh rows some footprint touches are cleared / read
+    // row occupancy (mode 2), plan-owned: bit (k N + j) of occ_cur = row j of plane k is touched by a
+    // footprint of the visibilities of the last rick_bin; occ_mesh = rows of the mesh that hold defined data
+    uint32_t *occ_cur_dev, *occ_mesh_dev;
+    uint32_t* row_list_dev;  // [Nw N] rows to clear, built by rick_grid
+    uint32_t* n_rows_dev;
     cufftHandle fft_rows;    // batched 1-D row transforms
     bool fft_rows_ready;
     size_t fft_rows_work_bytes;
@@ -152,3 +158,7 @@ int rick_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_f
 bool rick_colfft_supported(const rick_plan* p);
 int rick_colfft_init(rick_plan* p);
 int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
+int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st);          // rick_bin: occ_cur from the records
+int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st);   // rick_grid: clear new rows
+int rick_rows_list_all(rick_plan* p, cudaStream_t st);                   // row_list = all defined rows
+int rick_rowfft_impl(rick_plan* p, void* grid, cudaStream_t st);         // row transforms of the listed rows

@@ -1,0 +1,129 @@
+// rows.cu -- row occupancy of the mesh (rick_plan_set_fusion mode 2).
+//
+// The synthetic LOFAR-shaped workloads leave most (plane, row) pairs of the mesh untouched (60 % on config
+// 10M: the outer w-planes hold a few tracks each).  In fusion mode 2 the library keeps a bitmap of the rows
+// some footprint touches and spends memory traffic only on those: rick_grid clears only rows that are
+// touched and not yet defined, the fused column transform reads only defined rows (and takes zeros for the
+// others).  Untouched rows of the mesh hold undefined data in this mode.
+//   occ_cur   rows touched by the visibilities bound by the last rick_bin (rows j0-h .. j0+h of plane k)
+//   occ_mesh  rows that hold defined data (cleared or gridded) since the last rick_grid(zero_first != 0)
+#include "rick_internal.cuh"
+
+namespace {
+
+// one thread per sorted kept visibility: the first of every (plane, row j0) group sets the 2h+1 bits
+__global__ void __launch_bounds__(256) k_rows_mark(RickGeom g, const long long* __restrict__ n_kept,
+                                                   const uint2* __restrict__ ga, uint32_t* __restrict__ occ) {
+    const long long n = *n_kept;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint2 a = __ldg(ga + i);
+        const uint32_t j0 = a.x >> 16, k = a.y;
+        if (i > 0) {
+            const uint2 b = __ldg(ga + i - 1);
+            if ((b.x >> 16) == j0 && b.y == k) continue;
+        }
+        // rows j0-h .. j0+h as one or two word masks; bits only ever get set, so a plain (L2) read that
+        // already shows them saves the atomic: the many tiles of a mesh row would otherwise all hit one word
+        const uint32_t lo = k * (uint32_t)g.N + (j0 - (uint32_t)g.h), hi = lo + 2u * (uint32_t)g.h;
+        const uint32_t w0 = lo >> 5, w1 = hi >> 5;
+        const uint32_t span = (2u * (uint32_t)g.h + 1u);
+        const uint32_t m0 = (span >= 32u ? 0xffffffffu : ((1u << span) - 1u)) << (lo & 31);
+        if ((__ldcg(occ + w0) & m0) != m0) atomicOr(occ + w0, m0);
+        if (w1 != w0) {
+            const uint32_t m1 = (1u << ((hi & 31) + 1u)) - 1u;
+            if ((__ldcg(occ + w1) & m1) != m1) atomicOr(occ + w1, m1);
+        }
+    }
+}
+
+// all == 0: rows to clear = occ_cur & ~occ_mesh, as a list, and occ_mesh |= occ_cur;
+// all != 0: the list of all rows of occ_mesh (for the row transforms).  One CTA (the bitmap is small).
+__global__ void __launch_bounds__(1024) k_rows_new(int n_words, const uint32_t* __restrict__ occ_cur,
+                                                   uint32_t* __restrict__ occ_mesh, uint32_t* __restrict__ list,
+                                                   uint32_t* __restrict__ n_rows, int all) {
+    __shared__ uint32_t warp_tot[32];
+    __shared__ uint32_t base;
+    if (threadIdx.x == 0) base = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int w0 = 0; w0 < n_words; w0 += 1024) {
+        const int w = w0 + threadIdx.x;
+        uint32_t fresh = 0;
+        if (w < n_words) {
+            const uint32_t m = occ_mesh[w];
+            if (all) {
+                fresh = m;
+            } else {
+                const uint32_t c = occ_cur[w];
+                fresh = c & ~m;
+                occ_mesh[w] = m | c;
+            }
+        }
+        const uint32_t cnt = __popc(fresh);
+        uint32_t incl = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) warp_tot[warp] = incl;
+        __syncthreads();
+        uint32_t before = base;
+        for (int x = 0; x < warp; ++x) before += warp_tot[x];
+        uint32_t pos = before + incl - cnt;
+        while (fresh) {
+            const int b = __ffs(fresh) - 1;
+            fresh &= fresh - 1;
+            list[pos++] = (uint32_t)w * 32u + (uint32_t)b;
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) base = before + incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *n_rows = base;
+}
+
+// clear the listed rows (N cells of cell_bytes each)
+__global__ void __launch_bounds__(256) k_rows_zero(const uint32_t* __restrict__ list, const uint32_t* __restrict__ n_rows,
+                                                   uint4* __restrict__ grid, int row_vec /* 16-byte pieces per row */) {
+    const uint32_t n = *n_rows;
+    for (uint32_t r = blockIdx.x; r < n; r += gridDim.x) {
+        uint4* row = grid + (size_t)list[r] * row_vec;
+        for (int i = threadIdx.x; i < row_vec; i += 256) row[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
+}
+
+}  // namespace
+
+int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
+    const size_t words = (size_t)p->g.Nw * p->g.N / 32;
+    RICK_CUDA(cudaMemsetAsync(p->occ_cur_dev, 0, 4 * words, st));
+    if (M == 0) return RICK_OK;
+    const long long want = (M + 255) / 256;
+    const long long cap = (long long)p->sm_count * 16;
+    k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, p->grec_a, p->occ_cur_dev);
+    RICK_LAUNCH_CHECK();
+    p->launches++;
+    return RICK_OK;
+}
+
+int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st) {
+    const int words = (int)((size_t)p->g.Nw * p->g.N / 32);
+    if (zero_first) RICK_CUDA(cudaMemsetAsync(p->occ_mesh_dev, 0, 4 * (size_t)words, st));
+    k_rows_new<<<1, 1024, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 0);
+    RICK_LAUNCH_CHECK();
+    const int cell = (p->dtype == RICK_C128) ? 16 : 8;
+    k_rows_zero<<<p->sm_count * 8, 256, 0, st>>>(p->row_list_dev, p->n_rows_dev, (uint4*)grid, p->g.N * cell / 16);
+    RICK_LAUNCH_CHECK();
+    p->launches += 2;
+    return RICK_OK;
+}
+
+// list of all defined rows (for rick_fft_planes in fusion mode 2)
+int rick_rows_list_all(rick_plan* p, cudaStream_t st) {
+    const int words = (int)((size_t)p->g.Nw * p->g.N / 32);
+    k_rows_new<<<1, 1024, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 1);
+    RICK_LAUNCH_CHECK();
+    p->launches++;
+    return RICK_OK;
+}

@@ -323,3 +323,46 @@ def test_kaiser_bessel_kernel(name, M, plan, dtype, fused):
     gref = O.image(O.Plan(**pa), *hv)
     assert np.abs(img - gref)[inner, inner].max() > 10 * TOL[dtype] * peak
     im.close()
+
+
+@pytest.mark.parametrize("name,M,plan,kernel", [
+    ("10M", 400_000, dict(N=512, Nw=8), "gauss"),
+    ("10M", 1_000_003, dict(N=2048, Nw=32), "gauss"),
+    ("hotspot", 300_001, dict(N=1024, Nw=4), "kb"),
+])
+def test_fusion_mode_2_row_occupancy(name, M, plan, kernel):
+    """rick_plan_set_fusion(2): only the mesh rows some footprint touches are cleared and read.  The mesh is
+    pre-filled with NaN so that any read of an untouched row, or any touched row left uncleared, shows."""
+    cfg, vis, pa = make(name, M, dtype="c64", **plan)
+    N, beta = pa["N"], 2.34 * pa["support"]
+    im = B.Imager(dtype="c64", M_max=M, fused=2, kernel=kernel, beta=beta, **pa)
+    assert im.fused == 2
+    im.grid.fill_(complex(float("nan"), float("nan")))
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    oplan = O.Plan(kernel=kernel, beta=beta, **pa)
+    ref = O.image(oplan, *vis.numpy())
+    t = O.taper(N, cfg.support, cfg.sigma, kernel, beta)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    inner = slice(N // 4, 3 * N // 4)
+    peak = np.abs(ref[inner, inner]).max()
+    d = np.abs(img - ref)
+    assert np.isfinite(img).all()
+    a, b = d[tw >= 1e-2].max() / peak, (d * tw).max() / peak
+    print(f"mode2 {name} N={N} {kernel}: gateA {a:.2e} gateB {b:.2e}")
+    assert a <= TOL["c64"] and b <= TOL["c64"]
+    # again on the same (now dirty) mesh, and in two chunks with zero_first = 0 for the second
+    again = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    assert (np.abs(again - img) * tw).max() <= 2e-6 * np.abs(img * tw).max()
+    im.grid.fill_(complex(float("nan"), float("nan")))
+    half = vis.M // 2
+    for n, sl in enumerate((slice(0, half), slice(half, vis.M))):
+        im.bin(vis.u[sl].contiguous(), vis.v[sl].contiguous(), vis.w[sl].contiguous(), vis.vis[sl].contiguous(),
+               vis.weight[sl].contiguous())
+        im.grid_(zero_first=(n == 0))
+    im.fft()
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    chunked = im.image.cpu().numpy()
+    assert np.isfinite(chunked).all()
+    assert (np.abs(chunked - img) * tw).max() <= 2e-6 * np.abs(img * tw).max()
+    im.close()
