@@ -23,7 +23,10 @@ constexpr int kC = 4;            // columns per CTA
 constexpr int kT = 512;          // threads per CTA
 constexpr int kPadShift = 5;     // 4 float2 of padding after every 32 float2 (bank-conflict-free passes)
 
-__device__ __forceinline__ int padded(int idx) { return idx + ((idx >> kPadShift) << 2); }
+// X = 0: the column kernel's layout.  X = 2 (row kernel): two more slots after every 512, so that the last
+// pass can take its butterflies in frequency order (lanes 4 KB apart in the plain layout) at a 2-way conflict.
+template <int X = 0>
+__device__ __forceinline__ constexpr int padded(int idx) { return idx + ((idx >> kPadShift) << 2) + (idx >> 9) * X; }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
     return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
@@ -90,7 +93,7 @@ template <> __device__ __forceinline__ void dft<16>(float2* v) {
 //   x[B n + m + t n/R], t < R  ->  R-point DFT  ->  y_u * W_n^(m u) stored at the same slots (u for t).
 // tw[j] = exp(+2 pi i j / N).  Everything but m is a compile-time constant: the R slots of a butterfly
 // are the padded base plus constant offsets.
-template <int LOG2N, int R, int LOG2n>
+template <int LOG2N, int R, int LOG2n, int X = 0>
 __device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid) {
     constexpr int N = 1 << LOG2N, n = 1 << LOG2n;
     constexpr int q = n / R;                     // stride between the R inputs (rows)
@@ -98,18 +101,20 @@ __device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid)
     constexpr int per_block = stride;            // butterflies per sub-block = q * kC
     constexpr int total = N * kC / R;            // butterflies per pass
     constexpr int tw_step = N / n;
-    constexpr bool kConstOff = (stride % 32) == 0 || (R * stride <= 32);   // padding is affine over the butterfly
+    // the padding is affine over the butterfly when its slots step by whole padding groups, or stay inside one
+    constexpr bool kConstOff = (X == 0 ? (stride % 32) == 0 : ((stride % 512) == 0 || ((stride % 32) == 0 && R * stride <= 512))) ||
+                               (R * stride <= 32);
 #pragma unroll
     for (int w0 = 0; w0 < total; w0 += kT) {
         const int w = w0 + tid;
         if (total % kT != 0 && w >= total) break;
         const int B = w / per_block, rem = w % per_block;     // powers of two: shifts
         const int base = B * (n * kC) + rem;                  // ((B n + m) kC + c), rem = m kC + c
-        const int pb = padded(base);
+        const int pb = padded<X>(base);
         float2 v[R];
 #pragma unroll
         for (int t = 0; t < R; ++t)
-            v[t] = kConstOff ? buf[pb + t * (stride + ((stride >> kPadShift) << 2))] : buf[padded(base + t * stride)];
+            v[t] = kConstOff ? buf[pb + t * padded<X>(stride)] : buf[padded<X>(base + t * stride)];
         dft<R>(v);
         if (q > 1) {
             // W_n^(m u), u < R: the powers of two come from the table, the rest are products of at
@@ -129,8 +134,8 @@ __device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid)
         }
 #pragma unroll
         for (int u = 0; u < R; ++u) {
-            if (kConstOff) buf[pb + u * (stride + ((stride >> kPadShift) << 2))] = v[u];
-            else buf[padded(base + u * stride)] = v[u];
+            if (kConstOff) buf[pb + u * padded<X>(stride)] = v[u];
+            else buf[padded<X>(base + u * stride)] = v[u];
         }
     }
 }
@@ -153,7 +158,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
                                                            const float2* __restrict__ tw_g,
                                                            const double* __restrict__ inv_t,
                                                            double* __restrict__ image, int accumulate,
-                                                           const uint32_t* __restrict__ occ, int perm) {
+                                                           const uint32_t* __restrict__ occ) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 1 << LOG2N;
     constexpr int R3 = N >> 8;                        // radices 16 x 16 x R3
@@ -202,9 +207,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 #pragma unroll
     for (int e = 0; e < per_thread; ++e) {
         const int idx = owned_slot(e);
-        // perm: the rows were transformed by k_rowfft, which leaves column p at stored position s with
-        // p = slot_to_freq(s) (digit-reversed, never un-permuted)
-        const int q = slot_to_freq(idx / kC, N), sc = p0 + (idx % kC), p = perm ? slot_to_freq(sc, N) : sc;
+        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
         const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
         const double r2 = l * l + m * m;
         nm1r[e] = -r2 / (1.0 + sqrt(1.0 - r2));
@@ -252,7 +255,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 #pragma unroll
     for (int e = 0; e < per_thread; ++e) {
         const int idx = owned_slot(e);
-        const int q = slot_to_freq(idx / kC, N), sc = p0 + (idx % kC), p = perm ? slot_to_freq(sc, N) : sc;
+        const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
         const double sg = ((p + q) & 1) ? -1.0 : 1.0;
         double out = acc[e] * (sg * inv_t[q] * inv_t[p]);
         const size_t o = (size_t)q * N + p;
@@ -266,13 +269,14 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
 }
 
 // Row transforms of the listed mesh rows only (fusion mode 2), in place: four rows per step go through the
-// same shared-memory layout and DIF passes as four columns do in k_colfft_wcorrect; the result is written
-// back in the transform's own digit-reversed order (stored position s holds frequency slot_to_freq(s)):
-// the column kernel reads 4 stored-adjacent columns at a time and does not care which they are.
+// same shared-memory layout and DIF passes as four columns do in k_colfft_wcorrect; the last pass takes its
+// butterflies in frequency order and writes the rows back in natural order.
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+
+constexpr int kRowPad = 2;   // extra padding of the row kernel's layout (see padded<X>)
 
 template <int LOG2N>
 __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, const float2* __restrict__ tw_g,
@@ -281,7 +285,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
     constexpr int N = 1 << LOG2N;
     constexpr int R3 = N >> 8;
     constexpr int n_slots = N * kC;
-    constexpr int buf_elems = n_slots + ((n_slots >> kPadShift) << 2);
+    constexpr int buf_elems = padded<kRowPad>(n_slots);
     float2* buf0 = reinterpret_cast<float2*>(smem_raw);
     float2* buf1 = buf0 + buf_elems;
     float2* tw = buf1 + buf_elems;
@@ -294,7 +298,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
         for (int q = tid; q < N * kC; q += kT) {
             const int c = q >> LOG2N, i = q & (N - 1);
             const int r = grp * kC + c;
-            if (r < n) cp_async8(buf + padded(i * kC + c), planes + (size_t)list[r] * N + i);
+            if (r < n) cp_async8(buf + padded<kRowPad>(i * kC + c), planes + (size_t)list[r] * N + i);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -311,33 +315,26 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
         else asm volatile("cp.async.commit_group;" ::: "memory");
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncthreads();
-        dif_pass<LOG2N, 16, LOG2N>(buf, tw, tid);
+        dif_pass<LOG2N, 16, LOG2N, kRowPad>(buf, tw, tid);
         __syncthreads();
-        dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid);
+        dif_pass<LOG2N, 16, LOG2N - 4, kRowPad>(buf, tw, tid);
         __syncthreads();
-        if (R3 > 1) {
-            // last pass straight to global memory: butterfly (B, c) yields stored positions B R3 .. B R3 + R3 - 1 of row c
+        // Last pass straight to global memory, in NATURAL frequency order: the butterfly (u1, u2, c) holds
+        // frequencies u1 + 16 u2 + 256 u3, u3 < R3 (slots (u1 16 + u2) R3 + u3).  Lanes run over u1, so that
+        // every store instruction writes 16 consecutive frequencies of a row (full sectors).
 #pragma unroll
-            for (int bi = 0; bi < n_slots / kT / R3; ++bi) {
-                const int w = bi * kT + tid;
-                const int B = w / kC, c = w % kC;
-                const int pb = padded(B * (R3 * kC) + c);
-                float2 v[R3];
+        for (int bi = 0; bi < n_slots / kT / R3; ++bi) {
+            const int w = bi * kT + tid;
+            const int u1 = w & 15, c = (w >> 4) % kC, u2 = w / (16 * kC);
+            const int r = grp * kC + c;
+            float2 v[R3];
 #pragma unroll
-                for (int t = 0; t < R3; ++t) v[t] = buf[pb + t * kC];
-                dft<R3>(v);
-                const int r = grp * kC + c;
-                if (r < n) {
-                    float4* dst = reinterpret_cast<float4*>(planes + (size_t)list[r] * N + B * R3);
+            for (int t = 0; t < R3; ++t) v[t] = buf[padded<kRowPad>(((u1 * 16 + u2) * R3 + t) * kC + c)];
+            dft<R3>(v);
+            if (r < n) {
+                float2* dst = planes + (size_t)list[r] * N + (u1 + 16 * u2);
 #pragma unroll
-                    for (int u = 0; u < R3; u += 2) dst[u >> 1] = make_float4(v[u].x, v[u].y, v[u + 1].x, v[u + 1].y);
-                }
-            }
-        } else {
-            for (int q = tid; q < N * kC; q += kT) {
-                const int c = q >> LOG2N, i = q & (N - 1);
-                const int r = grp * kC + c;
-                if (r < n) planes[(size_t)list[r] * N + i] = buf[padded(i * kC + c)];
+                for (int u = 0; u < R3; ++u) dst[256 * u] = v[u];
             }
         }
         __syncthreads();                              // buf is free for the group after next
@@ -397,12 +394,11 @@ int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int
     const float2* tw = (const float2*)p->colfft_tw;
     const int acc = zero_first ? 0 : 1;
     const uint32_t* occ = p->fused == 2 ? p->occ_mesh_dev : nullptr;
-    const int perm = p->fused == 2 ? 1 : 0;
     switch (N) {
-        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
-        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
-        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
-        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, perm); break;
+        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
+        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
+        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
+        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
         default: return RICK_EINVAL;
     }
     RICK_LAUNCH_CHECK();
@@ -412,14 +408,14 @@ int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int
 
 int rick_rowfft_impl(rick_plan* p, void* grid, cudaStream_t st) {
     const int N = p->g.N;
-    const size_t smem = colfft_smem_bytes(N);
+    const size_t smem = colfft_smem_bytes(N) + 2 * (size_t)(N * kC / 512) * kRowPad * sizeof(float2);
     static bool attr_done = false;
     if (!attr_done) {
         const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
-        if (cudaFuncSetAttribute(k_rowfft<8>, a, (int)colfft_smem_bytes(256)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_rowfft<9>, a, (int)colfft_smem_bytes(512)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_rowfft<10>, a, (int)colfft_smem_bytes(1024)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_rowfft<11>, a, (int)colfft_smem_bytes(2048)) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_rowfft<8>, a, (int)(colfft_smem_bytes(256) + 2 * (256 * kC / 512) * kRowPad * sizeof(float2))) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<9>, a, (int)(colfft_smem_bytes(512) + 2 * (512 * kC / 512) * kRowPad * sizeof(float2))) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<10>, a, (int)(colfft_smem_bytes(1024) + 2 * (1024 * kC / 512) * kRowPad * sizeof(float2))) != cudaSuccess ||
+            cudaFuncSetAttribute(k_rowfft<11>, a, (int)(colfft_smem_bytes(2048) + 2 * (2048 * kC / 512) * kRowPad * sizeof(float2))) != cudaSuccess)
             return RICK_ECUDA;
         attr_done = true;
     }
