@@ -269,16 +269,21 @@ def main():
     stage_ms = {k: statistics.median(v) for k, v in per.items()}
     peak, peak_src = _peaks()
     _, n_pass, _ = B.rick_plan_sort_layout(im.plan)
+    # fusion mode 2 clears / transforms / reads only the mesh rows some footprint touches: those are the bytes
+    # the path needs; the dense-mesh figure of SURVEY.md section 8(d) is kept beside it for zero+grid
+    rows_total = cfg.Nw * cfg.N
+    rows_defined = B.rick_plan_rows_defined(im.plan) if im.fused == 2 else rows_total
+    live_bytes = mesh_bytes * rows_defined // rows_total
     alg = {   # algorithmic bytes per launch
         "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
         # sort: first pass 4 r + 8 w, middle passes 8 r + 8 w, last pass 8 r and, fused into it, the gather
         # (one 32-B record in, sorted SoA 24 B + gridder records 24 B out per kept visibility)
         "sort": ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept,
         "gather": 0,                                 # rides in the last sort pass (rick_bin without perm_out)
-        "zero": mesh_bytes,
+        "zero": live_bytes,
         "grid": 24 * n_kept,
-        "fft": (2 if im.fused else 4) * mesh_bytes,      # fused: row transforms only (one read + write)
-        "wcorrect": mesh_bytes + cfg.N * cfg.N * 8,      # fused: column transforms + screen + sum, one read
+        "fft": (2 if im.fused else 4) * live_bytes,      # fused: row transforms only (one read + write)
+        "wcorrect": live_bytes + cfg.N * cfg.N * 8,      # fused: column transforms + screen + sum, one read
     }
     stages = {}
     for k, b in alg.items():
@@ -291,7 +296,8 @@ def main():
     stages["zero+grid"] = {"ms": round(zg, 4), "alg_bytes": alg["zero"] + alg["grid"],
                            "gbs": (alg["zero"] + alg["grid"]) / (zg * 1e-3) / 1e9,
                            "frac": (alg["zero"] + alg["grid"]) / (zg * 1e-3) / 1e9 / peak,
-                           "vis_per_s": n_kept / (zg * 1e-3)}
+                           "vis_per_s": n_kept / (zg * 1e-3),
+                           "frac_dense_mesh_definition": (mesh_bytes + alg["grid"]) / (zg * 1e-3) / 1e9 / peak}
     # the dominant kernel = the library kernel with the largest total time in a step; its roofline numbers
     # are per launch (sort: n_pass launches of k_onesweep, the average pass)
     kernels = {"grid": ("k_grid_rec" if cfg.dtype == "c64" else "k_grid_runs", 1),
@@ -306,6 +312,21 @@ def main():
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": _traffic(kname), "peak_source": peak_src,
                 "launch_ms": launch_ms, "alg_bytes_per_launch": launch_bytes}
+    if kname == "k_colfft_wcorrect":
+        # the fused column transform is bound by fp32 instruction issue, not by HBM (profiles/): report it against
+        # the fp32 ALU peak DESIGN.md section 5 derives (148 SMs x 128 lanes x 2 flop x 1.965 GHz), with the
+        # 5 N log2 N flop of every column transform; the HBM view stays beside it
+        import math
+        flops = 5.0 * cfg.N * math.log2(cfg.N) * cfg.N * cfg.Nw
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        roofline = {"bound": "alu", "kernel": kname, "stage": dom, "launches_per_step": n_launch,
+                    "achieved": flops / (launch_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+                    "frac": flops / (launch_ms * 1e-3) / 1e12 / alu_peak,
+                    "traffic": _traffic(kname + ("_mode2" if im.fused == 2 else "")),
+                    "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 (FMA) x 1.965 GHz (DESIGN.md section 5)",
+                    "launch_ms": launch_ms, "alg_flops_per_launch": flops,
+                    "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                            "alg_bytes_per_launch": launch_bytes}}
 
     # end to end through rick_image_from_host: pinned host inputs -> host image, copies inside the region
     host = [x.cpu() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
@@ -336,7 +357,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
         "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
-                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype, "fusion_mode": int(im.fused),
+                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype, "fusion_mode": int(im.fused), "mesh_rows_defined": rows_defined, "mesh_rows": rows_total,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs (240 MB) and mesh (1.07 GB) exceed the 126 MB L2; no explicit flush"
                    if args.config == "10M" else "inputs and mesh exceed L2; no explicit flush"},

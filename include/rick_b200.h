@@ -100,6 +100,10 @@ int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
  * on = 0: off. */
 int rick_plan_set_fusion(rick_plan* plan, int on);
 
+/* Fusion mode 2 only: number of mesh rows (plane, j) that held defined data at the last rick_fft_planes
+ * (of Nw * N).  Host-synchronous.  RICK_ESTATE in other modes. */
+int rick_plan_rows_defined(rick_plan* plan, long long* rows);
+
 /* Sizes of the two caller-provided scratch buffers: `bin_bytes` for rick_bin with up to M
  * visibilities, `fft_bytes` for rick_fft_planes (0 if cuFFT needs none).  Either pointer may be NULL. */
 int rick_plan_workspace_bytes(const rick_plan* plan, long long M, size_t* bin_bytes, size_t* fft_bytes);

@@ -21,7 +21,7 @@ _lib = None
 
 EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
-    "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel",
+    "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
@@ -63,6 +63,7 @@ def lib():
         L.rick_plan_destroy.argtypes = [vp]
         L.rick_plan_set_fusion.argtypes = [vp, i]
         L.rick_plan_set_kernel.argtypes = [vp, i, dbl]
+        L.rick_plan_rows_defined.argtypes = [vp, C.POINTER(ll)]
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
@@ -137,6 +138,13 @@ def rick_plan_set_fusion(plan: int, on: int) -> int:
         return 0
     _check(rc, "rick_plan_set_fusion")
     return on
+
+
+def rick_plan_rows_defined(plan: int) -> int:
+    """Fusion mode 2: mesh rows that held defined data at the last rick_fft_planes."""
+    n = C.c_longlong()
+    _check(lib().rick_plan_rows_defined(plan, C.byref(n)), "rick_plan_rows_defined")
+    return int(n.value)
 
 
 RICK_KERNEL_GAUSS, RICK_KERNEL_KB = 0, 1

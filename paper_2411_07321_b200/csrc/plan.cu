@@ -342,6 +342,16 @@ int rick_plan_set_fusion(rick_plan* p, int on) {
     return RICK_OK;
 }
 
+int rick_plan_rows_defined(rick_plan* p, long long* rows) {
+    if (!p || !rows) return RICK_EINVAL;
+    if (p->fused != 2 || !p->n_rows_dev) return RICK_ESTATE;
+    uint32_t n = 0;
+    RICK_CUDA(cudaDeviceSynchronize());
+    RICK_CUDA(cudaMemcpy(&n, p->n_rows_dev, sizeof(n), cudaMemcpyDeviceToHost));
+    *rows = (long long)n;
+    return RICK_OK;
+}
+
 int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes, size_t* fft_bytes) {
     if (!p || M < 0 || M >= 4294967295ll) return RICK_EINVAL;
     if (bin_bytes) *bin_bytes = rick_bin_workspace_bytes(p, M);
