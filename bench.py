@@ -198,6 +198,8 @@ def main():
     ap.add_argument("--kernel", default="gauss", choices=["gauss", "kb"],
                     help="gridding kernel: the Gaussian of BASELINE.json (default) or the paper's Kaiser-Bessel (beta = 2.34 S)")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-chunks", type=int, default=4,
+                    help="time slices of rick_image_from_host_chunked in the e2e region (1: one copy, then compute)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -334,18 +336,24 @@ def main():
     if args.e2e_steps > 0:
         host = [x.pin_memory() for x in host]
         out = torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory()
-        im.run_from_host(*host, out)
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            im.run_from_host(*host, out)
-        torch.cuda.synchronize()
-        e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-        e2e_s = max_over_ranks(e2e_s, dist, dev)
+        def timed_from_host(chunks):
+            im.run_from_host(*host, out, chunks=chunks)
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                im.run_from_host(*host, out, chunks=chunks)
+            torch.cuda.synchronize()
+            return max_over_ranks((time.perf_counter() - t0) / args.e2e_steps, dist, dev)
+
+        e2e_s = timed_from_host(args.e2e_chunks)
         e2e = {"value": world * M / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
-               "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps}
+               "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps,
+               "chunks": args.e2e_chunks,
+               "call": "rick_image_from_host_chunked" if args.e2e_chunks > 1 else "rick_image_from_host"}
+        if args.e2e_chunks > 1:
+            e2e["ms_per_step_one_chunk"] = timed_from_host(1) * 1e3
 
     if rank != 0:
         if dist is not None:

@@ -177,6 +177,18 @@ int rick_image_from_host(rick_plan* plan, long long M, const float* u_host, cons
                          const float* w_host, const void* vis_host, const float* weight_host,
                          const rick_device_buffers* dev, double* image_host, void* stream);
 
+/* rick_image_from_host with the input split into n_chunks time slices ("the data are read and
+ * gridded in chunks"): the host-to-device copies of slice i+1 run on a second stream while slice i is binned
+ * and gridded onto the mesh (rick_grid with zero_first only for slice 0), then one rick_fft_planes,
+ * rick_wcorrect_accumulate and the image copy.  The staging arrays of `dev` (capacity M) are used as two
+ * halves, so a slice holds at most M/2 visibilities (rounded to a multiple of 1024); n_chunks < 2 or
+ * M < 2048 falls back to rick_image_from_host.  The image equals the single-slice one up to the order of
+ * the floating-point additions on the mesh.  Returns after synchronising `stream`. */
+int rick_image_from_host_chunked(rick_plan* plan, long long M, const float* u_host, const float* v_host,
+                                 const float* w_host, const void* vis_host, const float* weight_host,
+                                 const rick_device_buffers* dev, int n_chunks, double* image_host,
+                                 void* stream);
+
 /* CUDA-event times (milliseconds) of the most recent call of each stage, indexed by RICK_T_*;
  * stages never run report 0.  Synchronises on the recorded events.  n <= RICK_T_COUNT. */
 int rick_get_timings(rick_plan* plan, double* ms, int n);

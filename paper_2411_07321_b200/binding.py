@@ -23,7 +23,7 @@ EXPORTS = (
     "rick_plan_create", "rick_plan_set_dtype", "rick_plan_workspace_bytes", "rick_plan_destroy",
     "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
-    "rick_image_from_host", "rick_get_timings", "rick_launch_count", "rick_strerror",
+    "rick_image_from_host", "rick_image_from_host_chunked", "rick_get_timings", "rick_launch_count", "rick_strerror",
 )
 
 
@@ -71,6 +71,7 @@ def lib():
         L.rick_wcorrect_accumulate.argtypes = [vp, vp, vp, i, vp]
         L.rick_image.argtypes = [vp, vp, vp, i, vp]
         L.rick_image_from_host.argtypes = [vp, ll, vp, vp, vp, vp, vp, C.POINTER(_DeviceBuffers), vp, vp]
+        L.rick_image_from_host_chunked.argtypes = [vp, ll, vp, vp, vp, vp, vp, C.POINTER(_DeviceBuffers), i, vp, vp]
         L.rick_get_timings.argtypes = [vp, C.POINTER(dbl), i]
         L.rick_launch_count.argtypes = [vp]
         L.rick_launch_count.restype = ll
@@ -298,8 +299,9 @@ class Imager:
         self.wcorrect(True)
         return self.image
 
-    def run_from_host(self, u, v, w, vis, weight, image_host: torch.Tensor) -> torch.Tensor:
-        """rick_image_from_host: host (pinned) inputs -> host image, copies included."""
+    def run_from_host(self, u, v, w, vis, weight, image_host: torch.Tensor, chunks: int = 1) -> torch.Tensor:
+        """rick_image_from_host (chunks == 1) / rick_image_from_host_chunked: host (pinned) inputs -> host
+        image, copies included; with chunks > 1 the copies of one slice overlap the gridding of the last."""
         M = int(u.numel())
         self.reserve(M)
         if self.staging is None:
@@ -318,8 +320,13 @@ class Imager:
             _ptr(self.workspace), self.workspace.numel(), _ptr(self.grid),
             _ptr(self.fft_work), 0 if self.fft_work is None else self.fft_work.numel(),
             _ptr(self.image), _ptr(self.n_kept))
-        _check(lib().rick_image_from_host(self.plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight),
-                                          C.byref(b), _ptr(image_host), _stream()), "rick_image_from_host")
+        if chunks > 1:
+            _check(lib().rick_image_from_host_chunked(self.plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight),
+                                                      C.byref(b), int(chunks), _ptr(image_host), _stream()),
+                   "rick_image_from_host_chunked")
+        else:
+            _check(lib().rick_image_from_host(self.plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight),
+                                              C.byref(b), _ptr(image_host), _stream()), "rick_image_from_host")
         return image_host
 
     def timings(self) -> Dict[str, float]:

@@ -385,6 +385,11 @@ int rick_plan_destroy(rick_plan* p) {
         if (p->ev_start[i]) cudaEventDestroy(p->ev_start[i]);
         if (p->ev_stop[i]) cudaEventDestroy(p->ev_stop[i]);
     }
+    if (p->pipe_ready) {
+        cudaStreamDestroy(p->copy_stream);
+        for (int b = 0; b < 2; ++b) { cudaEventDestroy(p->ev_copied[b]); cudaEventDestroy(p->ev_consumed[b]); }
+        cudaEventDestroy(p->ev_entry);
+    }
     delete p;
     return RICK_OK;
 }
@@ -494,6 +499,73 @@ int rick_image_from_host(rick_plan* p, long long M, const float* u_h, const floa
                       NULL, NULL, NULL, d->workspace, d->workspace_bytes, d->n_kept, stream);
     if (rc != RICK_OK) return rc;
     if ((rc = rick_grid(p, d->grid, 1, stream)) != RICK_OK) return rc;
+    if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
+    if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
+    if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;
+    RICK_CUDA(cudaStreamSynchronize(st));
+    return RICK_OK;
+}
+
+static int pipe_init(rick_plan* p) {
+    if (p->pipe_ready) return RICK_OK;
+    RICK_CUDA(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming));
+        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
+    }
+    RICK_CUDA(cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
+    p->pipe_ready = true;
+    return RICK_OK;
+}
+
+int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, const float* v_h,
+                                 const float* w_h, const void* vis_h, const float* weight_h,
+                                 const rick_device_buffers* d, int n_chunks, double* image_host,
+                                 void* stream) {
+    if (!p || !d || !image_host || M < 0 || n_chunks < 1) return RICK_EINVAL;
+    if (n_chunks < 2 || M < 2 * 1024)
+        return rick_image_from_host(p, M, u_h, v_h, w_h, vis_h, weight_h, d, image_host, stream);
+    if (!u_h || !v_h || !w_h || !vis_h || !weight_h) return RICK_EINVAL;
+    int rc = pipe_init(p);
+    if (rc != RICK_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream, cs = p->copy_stream;
+    // chunk length: a multiple of 1024 visibilities, two of them within the staging capacity M
+    long long c = (M + n_chunks - 1) / n_chunks;
+    c = (c + 1023) / 1024 * 1024;
+    if (2 * c > M) c = M / 2 / 1024 * 1024;
+    const long long n = (M + c - 1) / c;
+    // the copy stream starts behind whatever `stream` holds (earlier users of the staging buffers)
+    RICK_CUDA(cudaEventRecord(p->ev_entry, st));
+    RICK_CUDA(cudaStreamWaitEvent(cs, p->ev_entry, 0));
+    auto copy_chunk = [&](long long i) -> int {
+        const int b = (int)(i & 1);
+        const size_t o = (size_t)(i * c), ob = (size_t)b * (size_t)c;
+        const size_t m = (size_t)((i + 1) * c <= M ? c : M - i * c);
+        if (i >= 2) RICK_CUDA(cudaStreamWaitEvent(cs, p->ev_consumed[b], 0));
+        RICK_CUDA(cudaMemcpyAsync(d->u + ob, u_h + o, 4 * m, cudaMemcpyHostToDevice, cs));
+        RICK_CUDA(cudaMemcpyAsync(d->v + ob, v_h + o, 4 * m, cudaMemcpyHostToDevice, cs));
+        RICK_CUDA(cudaMemcpyAsync(d->w + ob, w_h + o, 4 * m, cudaMemcpyHostToDevice, cs));
+        RICK_CUDA(cudaMemcpyAsync((char*)d->vis + 8 * ob, (const char*)vis_h + 8 * o, 8 * m,
+                                  cudaMemcpyHostToDevice, cs));
+        RICK_CUDA(cudaMemcpyAsync(d->weight + ob, weight_h + o, 4 * m, cudaMemcpyHostToDevice, cs));
+        RICK_CUDA(cudaEventRecord(p->ev_copied[b], cs));
+        return RICK_OK;
+    };
+    if ((rc = copy_chunk(0)) != RICK_OK) return rc;
+    for (long long i = 0; i < n; ++i) {
+        const int b = (int)(i & 1);
+        const size_t ob = (size_t)b * (size_t)c;
+        const long long m = (i + 1) * c <= M ? c : M - i * c;
+        // the next chunk's copies are queued before this chunk's kernels so that they overlap them
+        if (i + 1 < n && (rc = copy_chunk(i + 1)) != RICK_OK) return rc;
+        RICK_CUDA(cudaStreamWaitEvent(st, p->ev_copied[b], 0));
+        rc = rick_bin(p, m, d->u + ob, d->v + ob, d->w + ob, (char*)d->vis + 8 * ob, d->weight + ob, d->u_s,
+                      d->v_s, d->w_s, d->vis_s, d->weight_s, NULL, NULL, NULL, d->workspace,
+                      d->workspace_bytes, d->n_kept, stream);
+        if (rc != RICK_OK) return rc;
+        RICK_CUDA(cudaEventRecord(p->ev_consumed[b], st));   // rick_bin has read the staging half
+        if ((rc = rick_grid(p, d->grid, i == 0, stream)) != RICK_OK) return rc;
+    }
     if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
     if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
     if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;

@@ -81,6 +81,10 @@ struct rick_plan {
     const float2 *grec_b, *grec_c;
     // stage timing
     cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
+    // rick_image_from_host_chunked: copy stream and the events that hand the two staging halves back and forth
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_copied[2], ev_consumed[2], ev_entry;
+    bool pipe_ready;
     bool ev_valid[RICK_T_COUNT];
     long long launches;
     int sm_count;

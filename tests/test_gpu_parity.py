@@ -247,6 +247,31 @@ def test_chunked_accumulation_and_host_entry():
     assert (np.abs(out.numpy() - whole) * tw).max() <= 1e-12 * np.abs(whole * tw).max()
     tm = im.timings()
     assert all(tm[k] > 0 for k in ("bin", "zero", "grid", "fft", "wcorrect", "image"))
+    # rick_image_from_host_chunked: ragged slices (5 and 3 of them), copies on the second stream
+    for chunks in (5, 3, 2):
+        out.fill_(float("nan"))
+        im.run_from_host(*host, out, chunks=chunks)
+        assert (np.abs(out.numpy() - whole) * tw).max() <= 1e-12 * np.abs(whole * tw).max(), chunks
+    im.close()
+
+
+@pytest.mark.parametrize("fused", [0, 2])
+def test_image_from_host_chunked_c64(fused):
+    """rick_image_from_host_chunked on the c64 mesh, plain and with row occupancy (fusion mode 2):
+    the image of 7 time slices meets the oracle's gates; repeated calls reuse the staging halves."""
+    M = 700_001
+    cfg, vis, pa = make("10M", M, dtype="c64", N=512, Nw=8)
+    im = B.Imager(dtype="c64", M_max=M, fused=fused, **pa)
+    assert im.fused == fused
+    ref = O.image(O.Plan(**pa), *vis.numpy())
+    host = [x.cpu().pin_memory() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
+    out = torch.empty((pa["N"], pa["N"]), dtype=torch.float64).pin_memory()
+    for rep in range(3):
+        out.fill_(float("nan"))
+        im.grid.fill_(float("nan"))
+        im.run_from_host(*host, out, chunks=7)
+        a, b, full = gates(out.numpy(), ref, pa["N"], cfg.support, cfg.sigma)
+        assert a <= TOL["c64"] and b <= TOL["c64"], (rep, a, b, full)
     im.close()
 
 
