@@ -193,13 +193,18 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
         auto flush = [&]() {
             const int iw = kWin ? ((ci - h) & ~1) : (ci - h);   // first column of the window
             cell* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)iw;
+            cell* rowp[RB];                      // one address register pair per row (see k_grid_rec)
+#pragma unroll
+            for (int r = 0; r < RB; ++r) rowp[r] = base + (size_t)r * N;
+#pragma unroll
+            for (int r = 0; r < RB; ++r) asm volatile("" : "+l"(rowp[r]));
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
                     if constexpr (kWin) {
 #pragma unroll
                         for (int a = 0; a < W; a += 2) {
-                            float2* dst = (float2*)(base + (size_t)r * N + a);
+                            float2* dst = (float2*)(rowp[r] + a);
                             // the zero column may fall past the end of the row (only when i0 = N-1-h)
                             if (a + 2 == W && iw + W > (int)N)
                                 red_add_cell(dst, (float)ar[r][a], (float)ai[r][a]);
@@ -210,7 +215,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
                     } else {
 #pragma unroll
                         for (int a = 0; a < W; ++a) {
-                            red_add_cell(base + (size_t)r * N + a, ar[r][a], ai[r][a]);
+                            red_add_cell(rowp[r] + a, ar[r][a], ai[r][a]);
                             ar[r][a] = ai[r][a] = (real)0;
                         }
                     }
@@ -343,18 +348,37 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             const int iw = (int)(cij & 0xFFFFu), cj = (int)(cij >> 16);   // cij: window column | j0 << 16
             float2* base = grid + ((size_t)ck * N + (size_t)(cj - h + b0)) * N + (size_t)iw;
             const bool edge = iw + W > (int)N;      // the zero column would fall past the row (i0 = N-1-h)
+            // every row's address in a register pair of its own: a reduction holds its address register
+            // until the memory pipe has taken it, and reusing one pair for all rows stalled each row's
+            // address arithmetic behind the last row's reductions (27 % of the kernel's stall samples)
+            float2* rowp[RB];
 #pragma unroll
-            for (int r = 0; r < RB; ++r) {
-                if (b0 + r < S) {
+            for (int r = 0; r < RB; ++r) rowp[r] = base + (size_t)r * N;
 #pragma unroll
-                    for (int a = 0; a < W; a += 2) {
-                        float2* dst = base + (size_t)r * N + a;
-                        if (a + 2 == W && edge) red_add_cell(dst, ar[r][a], ai[r][a]);
-                        else red_add_pair(dst, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
-                        ar[r][a] = ai[r][a] = ar[r][a + 1] = ai[r][a + 1] = 0.f;
+            for (int r = 0; r < RB; ++r) asm volatile("" : "+l"(rowp[r]));
+            if (!edge) {
+#pragma unroll
+                for (int r = 0; r < RB; ++r)
+                    if (b0 + r < S) {
+#pragma unroll
+                        for (int a = 0; a < W; a += 2)
+                            red_add_pair(rowp[r] + a, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
                     }
-                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < RB; ++r)
+                    if (b0 + r < S) {
+#pragma unroll
+                        for (int a = 0; a < W; a += 2) {
+                            if (a + 2 == W) red_add_cell(rowp[r] + a, ar[r][a], ai[r][a]);
+                            else red_add_pair(rowp[r] + a, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
+                        }
+                    }
             }
+#pragma unroll
+            for (int r = 0; r < RB; ++r)
+#pragma unroll
+                for (int a = 0; a < W; ++a) ar[r][a] = ai[r][a] = 0.f;
         };
 
         auto one = [&](uint32_t ij, uint32_t k, float dx, float dy, float vr, float vi) {
