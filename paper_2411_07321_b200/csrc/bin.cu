@@ -11,6 +11,7 @@
 //                          read 8 B (4 B in the first pass: the index is implicit), write 8 B
 //   K3 gather              read 4 B index + one 32-B record (random rows), write 24 B
 #include "rick_internal.cuh"
+#include <type_traits>
 
 namespace {
 
@@ -223,35 +224,48 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
 
     uint32_t k[kSortItems], id[kSortItems];
     uint16_t rank[kSortItems];
-#pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
-        const long long gidx = base + j * 32;
-        const bool valid = gidx < M;
-        k[j] = valid ? __ldg(key_in + gidx) : 0u;
-        id[j] = kFirst ? (uint32_t)gidx : (valid ? __ldg(idx_in + gidx) : 0u);
-    }
     const unsigned lt = (1u << lane) - 1u;
+    const bool full = tile_base + kSortTile <= M;     // every tile but the last: no validity tests
+    // rank of an item among the items of its warp with the same digit (stable: lanes in order), by one
+    // ballot per digit bit; the warp's running count of the digit is kept by the lowest peer lane
+    auto rank_items = [&](auto full_c) {
+        constexpr bool kFull = decltype(full_c)::value;
 #pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
-        const bool valid = (base + j * 32) < M;
-        const uint32_t d = (k[j] >> shift) & mask;
-        unsigned peers = __ballot_sync(0xffffffffu, valid);
+        for (int j = 0; j < kSortItems; ++j) {
+            const long long gidx = base + j * 32;
+            const bool valid = kFull || gidx < M;
+            k[j] = valid ? __ldg(key_in + gidx) : 0u;
+            id[j] = kFirst ? (uint32_t)gidx : (valid ? __ldg(idx_in + gidx) : 0u);
+        }
 #pragma unroll
-        for (int b = 0; b < kBits; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const unsigned bal = __ballot_sync(0xffffffffu, bit);
-            peers &= bit ? bal : ~bal;
+        for (int j = 0; j < kSortItems; ++j) {
+            const bool valid = kFull || (base + j * 32) < M;
+            const uint32_t d = (k[j] >> shift) & mask;
+            unsigned peers = kFull ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+            for (int b = 0; b < kBits; ++b) {
+                unsigned m;      // lanes whose bit b equals this lane's
+                asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
+                    "and.b32 t, %1, %2;\n\t"
+                    "setp.ne.u32 p, t, 0;\n\t"
+                    "vote.sync.ballot.b32 %0, p, 0xffffffff;\n\t"
+                    "@!p not.b32 %0, %0;\n\t}"
+                    : "=r"(m) : "r"(d), "r"(1u << b));
+                peers &= m;
+            }
+            const int leader = __ffs(peers) - 1;   // valid lanes always contain themselves
+            uint32_t c = 0;
+            if (valid && lane == leader) {
+                c = sm.warp_cnt[warp][d];
+                sm.warp_cnt[warp][d] = c + (uint32_t)__popc(peers);
+            }
+            c = __shfl_sync(0xffffffffu, c, valid ? leader : lane);
+            rank[j] = (uint16_t)(c + (uint32_t)__popc(peers & lt));
+            __syncwarp();
         }
-        const int leader = __ffs(peers) - 1;   // valid lanes always contain themselves
-        uint32_t c = 0;
-        if (valid && lane == leader) {
-            c = sm.warp_cnt[warp][d];
-            sm.warp_cnt[warp][d] = c + (uint32_t)__popc(peers);
-        }
-        c = __shfl_sync(0xffffffffu, c, valid ? leader : lane);
-        rank[j] = (uint16_t)(c + (uint32_t)__popc(peers & lt));
-        __syncwarp();
-    }
+    };
+    if (full) rank_items(std::true_type{});
+    else rank_items(std::false_type{});
     __syncthreads();
 
     // per-digit totals over the warps (thread t owns digits 2t, 2t+1), exclusive offsets in place
@@ -304,32 +318,45 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
     // decoupled look-back: a window of kLookWin predecessors per digit is loaded at once (independent
     // loads in flight), then consumed from the nearest tile backwards up to the first inclusive prefix
     if (tile != 0) {
-        constexpr int kLookWin = 4;
+        // the digits of a thread walk back together, so that their polls are in flight at the same time
+        constexpr int kLookWin = 4 / kDigitsPerThread;
+        uint32_t excl[kDigitsPerThread];
+        long long t[kDigitsPerThread];
+        bool done[kDigitsPerThread];
+#pragma unroll
+        for (int q = 0; q < kDigitsPerThread; ++q) { excl[q] = 0; t[q] = (long long)tile - 1; done[q] = false; }
+        bool all_done = false;
+        while (!all_done) {
+            unsigned long long sv[kDigitsPerThread][kLookWin];
+#pragma unroll
+            for (int q = 0; q < kDigitsPerThread; ++q)
+#pragma unroll
+                for (int x = 0; x < kLookWin; ++x) {
+                    const long long tt = t[q] - x;
+                    sv[q][x] = (!done[q] && tt >= 0)
+                                   ? ld_status(status + (size_t)tt * kRadix + tid * kDigitsPerThread + q) : 0ull;
+                }
+            all_done = true;
+#pragma unroll
+            for (int q = 0; q < kDigitsPerThread; ++q) {
+#pragma unroll
+                for (int x = 0; x < kLookWin; ++x) {
+                    if (done[q] || t[q] < 0) continue;
+                    const unsigned long long v = sv[q][x];
+                    const bool ready = (uint32_t)((v >> 32) & 0x3FFFFFFFu) == epoch && (v >> 62) != 0ull;
+                    if (!ready) break;           // re-poll from this tile
+                    excl[q] += (uint32_t)v;
+                    if ((v >> 62) == 2ull || t[q] == 0) done[q] = true;
+                    --t[q];
+                }
+                all_done = all_done && done[q];
+            }
+        }
 #pragma unroll
         for (int q = 0; q < kDigitsPerThread; ++q) {
             const int d = tid * kDigitsPerThread + q;
-            uint32_t excl = 0;
-            long long t = (long long)tile - 1;
-            bool done = false;
-            while (!done) {
-                unsigned long long sv[kLookWin];
-#pragma unroll
-                for (int x = 0; x < kLookWin; ++x) {
-                    const long long tt = t - x;
-                    sv[x] = tt >= 0 ? ld_status(status + (size_t)tt * kRadix + d) : 0ull;
-                }
-#pragma unroll
-                for (int x = 0; x < kLookWin; ++x) {
-                    if (done || t < 0) continue;
-                    const bool ready = (uint32_t)((sv[x] >> 32) & 0x3FFFFFFFu) == epoch && (sv[x] >> 62) != 0ull;
-                    if (!ready) break;           // re-poll from this tile
-                    excl += (uint32_t)sv[x];
-                    if ((sv[x] >> 62) == 2ull || t == 0) done = true;
-                    --t;
-                }
-            }
-            st_status(status + (size_t)tile * kRadix + d, pack_status(2u, epoch, excl + tot[q]));
-            sm.glob[d] = digit_base[d] + excl - texcl[q];
+            st_status(status + (size_t)tile * kRadix + d, pack_status(2u, epoch, excl[q] + tot[q]));
+            sm.glob[d] = digit_base[d] + excl[q] - texcl[q];
         }
     } else {
 #pragma unroll
@@ -342,7 +369,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
     // exchange into digit order
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        const bool valid = (base + j * 32) < M;
+        const bool valid = full || (base + j * 32) < M;
         if (valid) {
             const uint32_t d = (k[j] >> shift) & mask;
             const uint32_t lp = sm.tile_excl[d] + sm.warp_cnt[warp][d] + rank[j];
