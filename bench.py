@@ -39,11 +39,13 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def _traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
+def _traffic(kernel: str, workload: str = "10M"):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary (captured on the
+    workload the file names), or None."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel)
+            d = json.load(f)
+            return d.get(kernel) if d.get("_workload", "10M") == workload else None
     except Exception:
         return None
 
@@ -312,7 +314,7 @@ def main():
     achieved = launch_bytes / (launch_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": kname, "stage": dom, "launches_per_step": n_launch,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": _traffic(kname), "peak_source": peak_src,
+                "traffic": _traffic(kname, args.config), "peak_source": peak_src,
                 "launch_ms": launch_ms, "alg_bytes_per_launch": launch_bytes}
     if kname == "k_colfft_wcorrect":
         # the fused column transform is bound by fp32 instruction issue, not by HBM (profiles/): report it against
@@ -324,7 +326,7 @@ def main():
         roofline = {"bound": "alu", "kernel": kname, "stage": dom, "launches_per_step": n_launch,
                     "achieved": flops / (launch_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
                     "frac": flops / (launch_ms * 1e-3) / 1e12 / alu_peak,
-                    "traffic": _traffic(kname + ("_mode2" if im.fused == 2 else "")),
+                    "traffic": _traffic(kname + ("_mode2" if im.fused == 2 else ""), args.config),
                     "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 (FMA) x 1.965 GHz (DESIGN.md section 5)",
                     "launch_ms": launch_ms, "alg_flops_per_launch": flops,
                     "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

@@ -38,49 +38,29 @@ __global__ void __launch_bounds__(256) k_rows_mark(RickGeom g, const long long* 
 }
 
 // all == 0: rows to clear = occ_cur & ~occ_mesh, as a list, and occ_mesh |= occ_cur;
-// all != 0: the list of all rows of occ_mesh (for the row transforms).  One CTA (the bitmap is small).
-__global__ void __launch_bounds__(1024) k_rows_new(int n_words, const uint32_t* __restrict__ occ_cur,
-                                                   uint32_t* __restrict__ occ_mesh, uint32_t* __restrict__ list,
-                                                   uint32_t* __restrict__ n_rows, int all) {
-    __shared__ uint32_t warp_tot[32];
-    __shared__ uint32_t base;
-    if (threadIdx.x == 0) base = 0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int w0 = 0; w0 < n_words; w0 += 1024) {
-        const int w = w0 + threadIdx.x;
-        uint32_t fresh = 0;
-        if (w < n_words) {
-            const uint32_t m = occ_mesh[w];
-            if (all) {
-                fresh = m;
-            } else {
-                const uint32_t c = occ_cur[w];
-                fresh = c & ~m;
-                occ_mesh[w] = m | c;
-            }
+// all != 0: the list of all rows of occ_mesh (for the row transforms).  One warp per bitmap word; the
+// words take their places in the list with one atomicAdd each on *n_rows (zeroed by the caller), so the
+// order of the list is arbitrary -- its users (k_rows_zero, k_rowfft) take the rows in any order.
+__global__ void __launch_bounds__(256) k_rows_new(int n_words, const uint32_t* __restrict__ occ_cur,
+                                                  uint32_t* __restrict__ occ_mesh, uint32_t* __restrict__ list,
+                                                  uint32_t* __restrict__ n_rows, int all) {
+    const int w = (int)blockIdx.x * 8 + (int)(threadIdx.x >> 5), lane = (int)(threadIdx.x & 31);
+    if (w >= n_words) return;
+    uint32_t fresh = 0, pos = 0;
+    if (lane == 0) {
+        const uint32_t m = occ_mesh[w];
+        if (all) {
+            fresh = m;
+        } else {
+            const uint32_t c = occ_cur[w];
+            fresh = c & ~m;
+            if (fresh) occ_mesh[w] = m | c;
         }
-        const uint32_t cnt = __popc(fresh);
-        uint32_t incl = cnt;
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += t;
-        }
-        if (lane == 31) warp_tot[warp] = incl;
-        __syncthreads();
-        uint32_t before = base;
-        for (int x = 0; x < warp; ++x) before += warp_tot[x];
-        uint32_t pos = before + incl - cnt;
-        while (fresh) {
-            const int b = __ffs(fresh) - 1;
-            fresh &= fresh - 1;
-            list[pos++] = (uint32_t)w * 32u + (uint32_t)b;
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) base = before + incl;
-        __syncthreads();
+        if (fresh) pos = atomicAdd(n_rows, (uint32_t)__popc(fresh));
     }
-    if (threadIdx.x == 0) *n_rows = base;
+    fresh = __shfl_sync(0xffffffffu, fresh, 0);
+    pos = __shfl_sync(0xffffffffu, pos, 0);
+    if ((fresh >> lane) & 1u) list[pos + (uint32_t)__popc(fresh & ((1u << lane) - 1u))] = (uint32_t)w * 32u + (uint32_t)lane;
 }
 
 // clear the listed rows (N cells of cell_bytes each)
@@ -110,7 +90,8 @@ int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
 int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st) {
     const int words = (int)((size_t)p->g.Nw * p->g.N / 32);
     if (zero_first) RICK_CUDA(cudaMemsetAsync(p->occ_mesh_dev, 0, 4 * (size_t)words, st));
-    k_rows_new<<<1, 1024, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 0);
+    RICK_CUDA(cudaMemsetAsync(p->n_rows_dev, 0, 4, st));
+    k_rows_new<<<(words + 7) / 8, 256, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 0);
     RICK_LAUNCH_CHECK();
     const int cell = (p->dtype == RICK_C128) ? 16 : 8;
     k_rows_zero<<<p->sm_count * 8, 256, 0, st>>>(p->row_list_dev, p->n_rows_dev, (uint4*)grid, p->g.N * cell / 16);
@@ -122,7 +103,8 @@ int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st) {
 // list of all defined rows (for rick_fft_planes in fusion mode 2)
 int rick_rows_list_all(rick_plan* p, cudaStream_t st) {
     const int words = (int)((size_t)p->g.Nw * p->g.N / 32);
-    k_rows_new<<<1, 1024, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 1);
+    RICK_CUDA(cudaMemsetAsync(p->n_rows_dev, 0, 4, st));
+    k_rows_new<<<(words + 7) / 8, 256, 0, st>>>(words, p->occ_cur_dev, p->occ_mesh_dev, p->row_list_dev, p->n_rows_dev, 1);
     RICK_LAUNCH_CHECK();
     p->launches++;
     return RICK_OK;
