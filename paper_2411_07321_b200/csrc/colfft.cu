@@ -158,7 +158,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
                                                            const float2* __restrict__ tw_g,
                                                            const double* __restrict__ inv_t,
                                                            double* __restrict__ image, int accumulate,
-                                                           const uint32_t* __restrict__ occ) {
+                                                           const uint32_t* __restrict__ occ, int col0) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 1 << LOG2N;
     constexpr int R3 = N >> 8;                        // radices 16 x 16 x R3
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
     float2* buf1 = buf0 + buf_elems;
     float2* tw = buf1 + buf_elems;                    // [N]
     const int tid = threadIdx.x;
-    const int p0 = blockIdx.x * kC;
+    const int p0 = col0 + blockIdx.x * kC;           // col0: first column of this launch's part of the image
     constexpr int per_thread = n_slots / kT;          // outputs owned by a thread: 2 .. 16
     // Ownership: with a third pass (R3 > 1) a thread keeps the R3 outputs of each of its last-pass
     // butterflies (entry e = bi R3 + u: butterfly w = bi kT + tid, sub-block B = w / kC, column c = w % kC,
@@ -380,25 +380,38 @@ int rick_colfft_init(rick_plan* p) {
     return RICK_OK;
 }
 
-int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st) {
+int rick_colfft_columns_per_cta() { return kC; }
+
+int rick_colfft_split(const rick_plan* p) {
+    // split the planes in two when that fills the last wave of CTAs better (one CTA per SM)
+    const int items = p->g.N / kC, sms = p->sm_count;
+    const double r1 = (double)((items + sms - 1) / sms), r2 = 0.5 * (double)((2 * items + sms - 1) / sms);
+    return (p->g.Nw >= 2 && r2 < 0.95 * r1) ? 2 : 1;
+}
+
+// Columns [col_lo, col_hi) of the image (multiples of kC = 4).  The whole image in one call, or part by part
+// (rick_image_from_host_chunked copies one part to the host while the next is computed); clear_image:
+// the plane halves of a split launch add onto a zeroed image -- zero it in the first part's call only.
+int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st,
+                              int col_lo, int col_hi, bool clear_image) {
     const RickGeom& g = p->g;
     const int N = g.N;
-    // split the planes in two when that fills the last wave of CTAs better (one CTA per SM)
-    const int items = N / kC, sms = p->sm_count;
-    const double r1 = (double)((items + sms - 1) / sms), r2 = 0.5 * (double)((2 * items + sms - 1) / sms);
-    const int ksplit = (g.Nw >= 2 && r2 < 0.95 * r1) ? 2 : 1;
-    if (ksplit > 1 && zero_first) RICK_CUDA(cudaMemsetAsync(image, 0, sizeof(double) * (size_t)N * N, st));
-    const dim3 blocks((unsigned)items, (unsigned)ksplit);
+    if (col_hi < 0) col_hi = N;
+    if (col_lo < 0 || col_hi > N || col_lo >= col_hi || (col_lo % kC) || (col_hi % kC)) return RICK_EINVAL;
+    const int ksplit = rick_colfft_split(p);
+    if (ksplit > 1 && zero_first && clear_image)
+        RICK_CUDA(cudaMemsetAsync(image, 0, sizeof(double) * (size_t)N * N, st));
+    const dim3 blocks((unsigned)((col_hi - col_lo) / kC), (unsigned)ksplit);
     const size_t smem = colfft_smem_bytes(N);
     const float2* planes = (const float2*)grid;
     const float2* tw = (const float2*)p->colfft_tw;
     const int acc = zero_first ? 0 : 1;
     const uint32_t* occ = p->fused == 2 ? p->occ_mesh_dev : nullptr;
     switch (N) {
-        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
-        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
-        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
-        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ); break;
+        case 256: k_colfft_wcorrect<8><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, col_lo); break;
+        case 512: k_colfft_wcorrect<9><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, col_lo); break;
+        case 1024: k_colfft_wcorrect<10><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, col_lo); break;
+        case 2048: k_colfft_wcorrect<11><<<blocks, kT, smem, st>>>(g, planes, tw, p->inv_taper_dev, image, acc, occ, col_lo); break;
         default: return RICK_EINVAL;
     }
     RICK_LAUNCH_CHECK();

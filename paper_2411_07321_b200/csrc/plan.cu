@@ -389,6 +389,7 @@ int rick_plan_destroy(rick_plan* p) {
         cudaStreamDestroy(p->copy_stream);
         for (int b = 0; b < 2; ++b) { cudaEventDestroy(p->ev_copied[b]); cudaEventDestroy(p->ev_consumed[b]); }
         cudaEventDestroy(p->ev_entry);
+        for (int i = 0; i < RICK_IMAGE_PARTS; ++i) cudaEventDestroy(p->ev_part[i]);
     }
     delete p;
     return RICK_OK;
@@ -514,6 +515,7 @@ static int pipe_init(rick_plan* p) {
         RICK_CUDA(cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
     }
     RICK_CUDA(cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
+    for (int i = 0; i < RICK_IMAGE_PARTS; ++i) RICK_CUDA(cudaEventCreateWithFlags(&p->ev_part[i], cudaEventDisableTiming));
     p->pipe_ready = true;
     return RICK_OK;
 }
@@ -567,9 +569,38 @@ int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, co
         if ((rc = rick_grid(p, d->grid, i == 0, stream)) != RICK_OK) return rc;
     }
     if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
-    if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
-    if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;
+    if (!p->fused) {
+        if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
+        if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;
+        RICK_CUDA(cudaStreamSynchronize(st));
+        return RICK_OK;
+    }
+    // fused column kernel: the image comes out in parts of whole waves of CTAs (two waves each, at most
+    // RICK_IMAGE_PARTS parts); the copy stream takes a part to the host while the next one is computed
+    const int N = p->g.N, kc = rick_colfft_columns_per_cta(), items = N / kc;
+    const int per_wave = p->sm_count / rick_colfft_split(p);          // column blocks per wave of CTAs
+    const int waves = (items + per_wave - 1) / per_wave;
+    int n_parts = (waves + 1) / 2;
+    n_parts = n_parts < 1 ? 1 : (n_parts > RICK_IMAGE_PARTS ? RICK_IMAGE_PARTS : n_parts);
+    const int waves_per_part = (waves + n_parts - 1) / n_parts;
+    {
+        StageTimer tm(p, RICK_T_WCORRECT, st);
+        int b_lo = 0;
+        for (int part = 0; part < n_parts && b_lo < items; ++part) {
+            int b_hi = b_lo + waves_per_part * per_wave;
+            if (b_hi > items || part == n_parts - 1) b_hi = items;
+            const int c_lo = b_lo * kc, c_hi = b_hi * kc;
+            if ((rc = rick_colfft_wcorrect_impl(p, d->grid, d->image, 1, st, c_lo, c_hi, part == 0)) != RICK_OK) return rc;
+            RICK_CUDA(cudaEventRecord(p->ev_part[part], st));
+            RICK_CUDA(cudaStreamWaitEvent(cs, p->ev_part[part], 0));
+            RICK_CUDA(cudaMemcpy2DAsync(image_host + c_lo, sizeof(double) * (size_t)N, d->image + c_lo,
+                                        sizeof(double) * (size_t)N, sizeof(double) * (size_t)(c_hi - c_lo), (size_t)N,
+                                        cudaMemcpyDeviceToHost, cs));
+            b_lo = b_hi;
+        }
+    }
     RICK_CUDA(cudaStreamSynchronize(st));
+    RICK_CUDA(cudaStreamSynchronize(cs));
     return RICK_OK;
 }
 

@@ -11,6 +11,7 @@
 #define RICK_TILE 32          // uv tile edge of the sort key (BASELINE.json north_star (2))
 #define RICK_MAX_PASSES 4
 #define RICK_KB_POLY_TERMS 10
+#define RICK_IMAGE_PARTS 4            // rick_image_from_host_chunked: image parts copied out while the next is computed
 #define RICK_GREC_PAD 4096    // gridder records are allocated in whole chunks of this many (one CTA's share)
 #define RICK_RADIX_BITS_MAX 9
 
@@ -83,7 +84,7 @@ struct rick_plan {
     cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
     // rick_image_from_host_chunked: copy stream and the events that hand the two staging halves back and forth
     cudaStream_t copy_stream;
-    cudaEvent_t ev_copied[2], ev_consumed[2], ev_entry;
+    cudaEvent_t ev_copied[2], ev_consumed[2], ev_entry, ev_part[RICK_IMAGE_PARTS];
     bool pipe_ready;
     bool ev_valid[RICK_T_COUNT];
     long long launches;
@@ -161,7 +162,10 @@ int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st);
 int rick_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
 bool rick_colfft_supported(const rick_plan* p);
 int rick_colfft_init(rick_plan* p);
-int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
+int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st,
+                              int col_lo = 0, int col_hi = -1, bool clear_image = true);
+int rick_colfft_split(const rick_plan* p);                              // 1 or 2 plane halves per column block
+int rick_colfft_columns_per_cta();
 int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st);          // rick_bin: occ_cur from the records
 int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st);   // rick_grid: clear new rows
 int rick_rows_list_all(rick_plan* p, cudaStream_t st);                   // row_list = all defined rows

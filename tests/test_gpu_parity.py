@@ -255,12 +255,17 @@ def test_chunked_accumulation_and_host_entry():
     im.close()
 
 
-@pytest.mark.parametrize("fused", [0, 2])
-def test_image_from_host_chunked_c64(fused):
+@pytest.mark.parametrize("fused,M,plan", [
+    (0, 700_001, dict(N=512, Nw=8)),
+    (2, 700_001, dict(N=512, Nw=8)),
+    (1, 1_000_003, dict(N=2048, Nw=32)),       # the bench plan: the image leaves in four parts
+    (2, 1_000_003, dict(N=2048, Nw=32)),
+])
+def test_image_from_host_chunked_c64(fused, M, plan):
     """rick_image_from_host_chunked on the c64 mesh, plain and with row occupancy (fusion mode 2):
-    the image of 7 time slices meets the oracle's gates; repeated calls reuse the staging halves."""
-    M = 700_001
-    cfg, vis, pa = make("10M", M, dtype="c64", N=512, Nw=8)
+    the image of 7 time slices meets the oracle's gates; repeated calls reuse the staging halves; with the
+    fused column kernel the image is copied out part by part while the next part is computed."""
+    cfg, vis, pa = make("10M", M, dtype="c64", **plan)
     im = B.Imager(dtype="c64", M_max=M, fused=fused, **pa)
     assert im.fused == fused
     ref = O.image(O.Plan(**pa), *vis.numpy())
