@@ -186,11 +186,25 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         const float2* src = planes + (size_t)k * N * N + p0;
         // row j: kC float2 = 32 B = two 16-byte pieces.  Fusion mode 2 (occ != NULL): rows no footprint
         // touched hold undefined data and are not read -- their slots are zero-filled instead.
-        for (int q = tid; q < N * 2; q += kT) {
-            const int j = q >> 1, half = q & 1;
+        // A warp's 32 pieces of one iteration are 16 consecutive rows, all in one word of the bitmap: lane
+        // `it` fetches the word of iteration `it` (one load per lane, all in flight together) and the
+        // iterations take theirs by shuffle.  (One dependent load per iteration cost 8 % of the kernel.)
+        constexpr int kIt = N * 2 / kT;
+        static_assert(kIt <= 32 && (kT / 2) % 32 == 0, "one bitmap word per warp and iteration");
+        uint32_t live = 0xFFFFFFFFu;
+        if (occ) {
+            const int lane = tid & 31, row0 = (tid & ~31) >> 1;          // first row of the warp, iteration 0
+            const uint32_t wv = lane < kIt ? __ldg(occ + ((k * N + row0 + lane * (kT / 2)) >> 5)) : 0u;
+            live = 0;
+#pragma unroll
+            for (int it = 0; it < kIt; ++it)
+                live |= ((__shfl_sync(0xffffffffu, wv, it) >> ((row0 + (lane >> 1)) & 31)) & 1u) << it;
+        }
+#pragma unroll 1
+        for (int it = 0; it < kIt; ++it) {
+            const int q = tid + it * kT, j = q >> 1, half = q & 1;
             float2* dst = buf + padded(j * kC + half * 2);
-            const bool live = !occ || ((__ldg(occ + ((k * N + j) >> 5)) >> (j & 31)) & 1u);
-            if (live) cp_async16(dst, src + (size_t)j * N + half * 2);
+            if ((live >> it) & 1u) cp_async16(dst, src + (size_t)j * N + half * 2);
             else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
