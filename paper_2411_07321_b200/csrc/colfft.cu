@@ -309,10 +309,19 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
 
     auto issue = [&](int grp, float2* buf) {
         // slot (i, c) <- element i of row list[4 grp + c]; consecutive threads take consecutive i (coalesced)
-        for (int q = tid; q < N * kC; q += kT) {
+        // (the group's row numbers are fetched before the copies: the copies clobber memory as far as the
+        // compiler knows, and one dependent load per copy iteration is what cost K6 8 %)
+        uint32_t row[kC];
+#pragma unroll
+        for (int c = 0; c < kC; ++c) row[c] = (grp * kC + c < n) ? __ldg(list + grp * kC + c) : 0xFFFFFFFFu;
+#pragma unroll
+        for (int it = 0; it < N * kC / kT; ++it) {
+            const int q = tid + it * kT;
             const int c = q >> LOG2N, i = q & (N - 1);
-            const int r = grp * kC + c;
-            if (r < n) cp_async8(buf + padded<kRowPad>(i * kC + c), planes + (size_t)list[r] * N + i);
+            uint32_t rw = row[0];
+#pragma unroll
+            for (int x = 1; x < kC; ++x) rw = (c == x) ? row[x] : rw;
+            if (rw != 0xFFFFFFFFu) cp_async8(buf + padded<kRowPad>(i * kC + c), planes + (size_t)rw * N + i);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
