@@ -12,9 +12,10 @@
 // The transformed planes are never written back: the column pass of a 2-D FFT (read + write of the
 // mesh) and the K5 sweep (another read) collapse into one read.
 //
-// Phase: w_k * nm1 reduced to [-1/2, 1/2] turns in fp64 (nm1 of a thread's pixels kept in registers), then the
-// hardware sine / cosine in fp32 on the reduced argument (abs error < 5e-7, the precision of the fp32
-// planes themselves); the product in fp32, the plane sum in fp64.
+// Phase: w_k * nm1 in fp64 (nm1 of a thread's pixels kept in registers), its fraction rounded to 2^-23 turns
+// (3.7e-7 rad at worst) and reduced to [-1/2, 1/2), then the hardware sine / cosine in fp32 on the reduced
+// argument (abs error < 5e-7, the precision of the fp32 planes themselves); the product in fp32, the plane
+// sum in fp64.
 #include "rick_internal.cuh"
 
 namespace {
@@ -228,10 +229,15 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         acc[e] = 0.0;
     }
     auto screen_add = [&](int e, float2 v, double wk) {
-        double t = wk * nm1r[e];
-        t -= rint(t);                                          // [-1/2, 1/2] turns
+        // fraction of w_k nm1 in fixed point, without the conversion pipe (rint and the fp64 -> fp32 narrowing
+        // are XU instructions, 4 lanes per clock and scheduler: with the two MUFUs and the widening below they
+        // made the screen XU-bound): adding 1.5 * 2^29 rounds the product (one DFMA) to 2^-23 turns and leaves
+        // the fraction, two's complement, in the low 23 mantissa bits (|w_k nm1| < 2^28 turns).
+        const double z = fma(wk, nm1r[e], 805306368.0);
+        const float gq = __int_as_float(0x3F800000 | (__double2loint(z) & 0x007FFFFF));   // 1 + fraction
+        const float t = gq - (gq >= 1.5f ? 2.0f : 1.0f);       // [-1/2, 1/2) turns, exact
         float sn, cs;
-        __sincosf(6.283185307179586f * (float)t, &sn, &cs);    // MUFU on [-pi, pi]: abs error < 5e-7
+        __sincosf(6.283185307179586f * t, &sn, &cs);           // MUFU on [-pi, pi]: abs error < 5e-7
         acc[e] += (double)(cs * v.x - sn * v.y);
     };
 
