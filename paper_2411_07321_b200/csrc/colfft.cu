@@ -94,8 +94,11 @@ template <> __device__ __forceinline__ void dft<16>(float2* v) {
 //   x[B n + m + t n/R], t < R  ->  R-point DFT  ->  y_u * W_n^(m u) stored at the same slots (u for t).
 // tw[j] = exp(+2 pi i j / N).  Everything but m is a compile-time constant: the R slots of a butterfly
 // are the padded base plus constant offsets.
+// In the second pass (n = N/16) a warp holds only N/256 <= 8 distinct m, and their table entries lie
+// 128 u bytes apart -- all in one bank (4 wavefronts per load, 12 % of the kernel's shared-memory wavefronts).
+// That pass reads a compact copy instead: tw2[ui q + m] = W_n^(m 2^ui), q = N/256 consecutive entries per power.
 template <int LOG2N, int R, int LOG2n, int X = 0>
-__device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid) {
+__device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid, const float2* tw2 = nullptr) {
     constexpr int N = 1 << LOG2N, n = 1 << LOG2n;
     constexpr int q = n / R;                     // stride between the R inputs (rows)
     constexpr int stride = q * kC;               // ... in float2 slots
@@ -122,8 +125,13 @@ __device__ __forceinline__ void dif_pass(float2* buf, const float2* tw, int tid)
             // most three of them (shared-memory bandwidth, not arithmetic, bounds this kernel)
             const int ts = (rem / kC) * tw_step;              // m * N / n
             float2 wp[R];
+            if (LOG2n == LOG2N - 4 && R == 16) {
 #pragma unroll
-            for (int u = 1; u < R; u <<= 1) wp[u] = tw[(ts * u) & (N - 1)];
+                for (int ui = 0; ui < 4; ++ui) wp[1 << ui] = tw2[ui * q + rem / kC];
+            } else {
+#pragma unroll
+                for (int u = 1; u < R; u <<= 1) wp[u] = tw[(ts * u) & (N - 1)];
+            }
 #pragma unroll
             for (int u = 3; u < R; ++u)
                 if (u & (u - 1)) {                            // not a power of two: lowest set bit times the rest
@@ -168,6 +176,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
     float2* buf0 = reinterpret_cast<float2*>(smem_raw);
     float2* buf1 = buf0 + buf_elems;
     float2* tw = buf1 + buf_elems;                    // [N]
+    float2* tw2 = tw + N;                             // [4 R3] second-pass twiddles, compact
     const int tid = threadIdx.x;
     const int p0 = col0 + blockIdx.x * kC;           // col0: first column of this launch's part of the image
     constexpr int per_thread = n_slots / kT;          // outputs owned by a thread: 2 .. 16
@@ -218,6 +227,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
     if (k_lo >= k_hi) return;
     issue(k_lo, buf0);
     for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
+    for (int i = tid; i < 4 * R3; i += kT) tw2[i] = tw_g[(((i % R3) * 16) << (i / R3)) & (N - 1)];
     double acc[per_thread], nm1r[per_thread];         // plane sum and n - 1 of the owned pixels
 #pragma unroll
     for (int e = 0; e < per_thread; ++e) {
@@ -250,7 +260,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         __syncthreads();
         dif_pass<LOG2N, 16, LOG2N>(buf, tw, tid);
         __syncthreads();
-        dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid);
+        dif_pass<LOG2N, 16, LOG2N - 4>(buf, tw, tid, tw2);
         __syncthreads();
         const double wk = g.w_min + ((double)k + 0.5) * g.dw;
         if (R3 > 1) {
@@ -309,6 +319,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
     float2* buf0 = reinterpret_cast<float2*>(smem_raw);
     float2* buf1 = buf0 + buf_elems;
     float2* tw = buf1 + buf_elems;
+    float2* tw2 = tw + N;
     const int tid = threadIdx.x;
     const int n = (int)*n_rows;
     const int n_groups = (n + kC - 1) / kC;
@@ -336,6 +347,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
     if (grp >= n_groups) return;
     issue(grp, buf0);
     for (int i = tid; i < N; i += kT) tw[i] = tw_g[i];
+    for (int i = tid; i < 4 * R3; i += kT) tw2[i] = tw_g[(((i % R3) * 16) << (i / R3)) & (N - 1)];
     int par = 0;
     for (; grp < n_groups; grp += gridDim.x, par ^= 1) {
         float2* buf = par ? buf1 : buf0;
@@ -346,7 +358,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
         __syncthreads();
         dif_pass<LOG2N, 16, LOG2N, kRowPad>(buf, tw, tid);
         __syncthreads();
-        dif_pass<LOG2N, 16, LOG2N - 4, kRowPad>(buf, tw, tid);
+        dif_pass<LOG2N, 16, LOG2N - 4, kRowPad>(buf, tw, tid, tw2);
         __syncthreads();
         // Last pass straight to global memory, in NATURAL frequency order: the butterfly (u1, u2, c) holds
         // frequencies u1 + 16 u2 + 256 u3, u3 < R3 (slots (u1 16 + u2) R3 + u3).  Lanes run over u1, so that
@@ -373,7 +385,7 @@ __global__ void __launch_bounds__(kT, 1) k_rowfft(float2* __restrict__ planes, c
 size_t colfft_smem_bytes(int N) {
     const int n_slots = N * kC;
     const size_t buf = (size_t)(n_slots + ((n_slots >> kPadShift) << 2)) * sizeof(float2);
-    return 2 * buf + (size_t)N * sizeof(float2);
+    return 2 * buf + (size_t)(N + 32) * sizeof(float2);      // + twiddles + compact second-pass twiddles
 }
 
 }  // namespace
