@@ -79,13 +79,27 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
     unsigned kept = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
     // warp-uniform trip count so that every lane reaches the votes
+    // the loads of the next trip are issued before this trip's arithmetic and votes (twice the bytes in
+    // flight per thread: the kernel waits on DRAM latency, not on bandwidth)
+    float uu = 0.f, vv = 0.f, ww = 0.f, wgt = 0.f;
+    float2 vi = make_float2(0.f, 0.f);
+    {
+        const long long m0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (m0 < M) { uu = __ldg(u + m0); vv = __ldg(v + m0); ww = __ldg(w + m0); wgt = __ldg(wt + m0); vi = __ldg(vis + m0); }
+    }
     for (long long base = (long long)blockIdx.x * blockDim.x; base < M; base += stride) {
         const long long m = base + threadIdx.x;
         const bool valid = m < M;
         uint32_t kk = 0;
+        const float uu_c = uu, vv_c = vv, ww_c = ww, wgt_c = wgt;
+        const float2 vi_c = vi;
+        if (m + stride < M) {
+            const long long mn = m + stride;
+            uu = __ldg(u + mn); vv = __ldg(v + mn); ww = __ldg(w + mn); wgt = __ldg(wt + mn); vi = __ldg(vis + mn);
+        }
         if (valid) {
-            const float uu = __ldg(u + m), vv = __ldg(v + m), ww = __ldg(w + m), wgt = __ldg(wt + m);
-            const float2 vi = __ldg(vis + m);
+            const float uu = uu_c, vv = vv_c, ww = ww_c, wgt = wgt_c;
+            const float2 vi = vi_c;
             RickLoc r = rick_locate(g, uu, vv, ww);
             const bool fin = rick_finite(uu) && rick_finite(vv) && rick_finite(ww) && rick_finite(wgt) &&
                              rick_finite(vi.x) && rick_finite(vi.y);
