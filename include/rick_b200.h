@@ -89,7 +89,7 @@ int rick_plan_set_dtype(rick_plan* plan, int dtype);
  * Errors: RICK_EINVAL (unknown kind, beta <= 0 or > 64), RICK_ENOMEM, RICK_ECUDA. */
 int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
 
-/* Fused column transform (optional; RICK_C64 and N in {256, 512, 1024, 2048} only, RICK_EINVAL otherwise;
+/* Fused column transform (optional; RICK_C64, N in {256, 512, 1024, 2048} and |w| < 2^28 wavelengths only, RICK_EINVAL otherwise;
  * call after rick_plan_set_dtype, which switches it off, and before rick_bin).
  * on = 1: rick_fft_planes runs only the row transforms of D7 (the mesh then holds row-transformed planes),
  * and rick_wcorrect_accumulate performs the column transforms itself, fused with the phase screen, the plane

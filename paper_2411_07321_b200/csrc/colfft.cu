@@ -392,7 +392,10 @@ size_t colfft_smem_bytes(int N) {
 
 bool rick_colfft_supported(const rick_plan* p) {
     const int N = p->g.N;
-    return p->dtype == RICK_C64 && (N == 256 || N == 512 || N == 1024 || N == 2048);
+    // the screen takes the fraction of w_k nm1 (|nm1| < 1) from the low mantissa bits of w_k nm1 + 1.5 * 2^29:
+    // |w| must stay below 2^28 wavelengths (2.7e8; the longest baselines on Earth are ~1e7 at 1 GHz)
+    const double w_abs = fmax(fabs(p->g.w_min), fabs(p->g.w_max));
+    return p->dtype == RICK_C64 && (N == 256 || N == 512 || N == 1024 || N == 2048) && w_abs < 268435456.0;
 }
 
 int rick_colfft_init(rick_plan* p) {

@@ -311,6 +311,11 @@ def test_fused_column_transform(name, M, plan):
     im2 = B.Imager(dtype="c128", M_max=16, fused=True, **pa)
     assert not im2.fused
     im2.close()
+    # so does a plan whose |w| reaches 2^28 wavelengths (the fused screen's fixed-point phase fraction)
+    pa3 = dict(pa, w_min=-1.0, w_max=float(2 ** 28))
+    im3 = B.Imager(dtype="c64", M_max=16, fused=True, **pa3)
+    assert not im3.fused
+    im3.close()
 
 
 @pytest.mark.parametrize("name,M,plan,dtype,fused", [
