@@ -19,8 +19,9 @@
  *   - Every function returns RICK_OK (0) or a negative rick_status; nothing throws or exits.
  *   - "device" pointers are CUDA device pointers on the current device, "host" pointers are host memory.
  *     The caller owns every buffer it passes; the library owns only the plan (geometry constants, the
- *     1-D taper table, the cuFFT handle, stage-timing events).  No allocation happens after
- *     rick_plan_create / rick_plan_set_dtype.
+ *     1-D taper table, the cuFFT handle, stage-timing events, the copy stream and hand-over events of
+ *     rick_image_from_host_chunked).  Allocation happens only in the rick_plan_* calls (create, set_dtype,
+ *     set_kernel, set_fusion); the path calls (rick_bin ... rick_image_from_host_chunked) allocate nothing.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
  *     enqueued asynchronously on it unless stated otherwise.
  *   - Geometry [D1]: du = 1/(N dl).  Mesh node i <-> u = (i - N/2) du; pixel p <-> l = (p - N/2) dl.
@@ -69,7 +70,7 @@ enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_
  *   N        mesh and image size per axis; a multiple of 32 (tile size), 32 <= N <= 32768
  *   Nw       number of w-planes, 1 <= Nw <= 4096, Nw (N/32)^2 <= 2^27
  *   support  full footprint width S in cells, odd, 3 <= S <= 15  (h = (S-1)/2)
- *   sigma    Gaussian width in cells, > 0
+ *   sigma    Gaussian width in cells, >= 0.25 (narrower kernels are refused: RICK_EINVAL)
  *   w_min, w_max   w range covered by the Nw planes, w_max > w_min; plane k is centred at
  *            w_min + (k + 1/2)(w_max - w_min)/Nw  [D3]
  *   dl       pixel size (direction cosine per pixel), > 0, N dl < sqrt(2)

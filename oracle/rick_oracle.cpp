@@ -309,34 +309,30 @@ long long rick_oracle_keys(int N, int Nw, int S, double w_min, double w_max, dou
     return kept;
 }
 
-// D4': the key rick_bin actually sorts by is the tile key of D4 refined by the
-// in-tile cell index c = (j0 & 31) * 32 + (i0 & 31) (10 bits), so that visibilities sharing a nearest
-// cell are adjacent while the order stays grouped by (plane, tile):
-//     cb       = the largest c <= 10 with  Nw T^2 * 2^c <= 2^32
-//     sort_key = key * 2^cb + (c >> (10 - cb))          kept visibilities
-//     sort_key = Nw T^2 * 2^cb - 1                        dropped visibilities: the largest key, which belongs to
-//                row j0 = N - 1 of the last tile (cb >= 5 keeps all of j0 & 31; Nw T^2 <= 2^27 is required)
-//                and is never kept by D5 since h >= 1; so dropped visibilities sort last, after every kept one
-// key / i0 / j0 are the outputs of rick_oracle_keys.  Returns cb.
-int rick_oracle_sort_key(int N, int Nw, long long M, const uint32_t* key, const int32_t* i0,
-                         const int32_t* j0, uint32_t* sort_key) {
-    const uint64_t T = (uint64_t)(N / 32);
-    const uint64_t n_bins = (uint64_t)Nw * T * T;
-    int cb = 10;
-    while (cb > 0 && (n_bins << cb) > (1ull << 32)) --cb;
-    const uint32_t sentinel = (uint32_t)((n_bins << cb) - 1);
-    for (long long m = 0; m < M; ++m) {
-        if ((uint64_t)key[m] >= n_bins) {
-            sort_key[m] = sentinel;
-        } else {
-            const uint64_t c = (uint64_t)(((j0[m] & 31) << 5) | (i0[m] & 31));
-            sort_key[m] = (uint32_t)(((uint64_t)key[m] << cb) | (c >> (10 - cb)));
-        }
-    }
-    return cb;
+// D4': the order rick_bin leaves the visibilities in.  BASELINE.json north_star (2) asks
+// for a sort by (w-plane, 32x32 uv tile); D4' refines it so that visibilities sharing a nearest cell are
+// adjacent: kept visibilities first, ordered by
+//     w-plane k,  tile row j0 / 32,  tile column i0 / 32,  row inside the tile j0 % 32,
+//     column inside the tile (i0 % 32) / 2^col_drop,  input index (the sort is stable);
+// dropped visibilities (k < 0) follow, in input order.  col_drop = 0 (the exact cell) for every plan with
+// Nw (N/32)^2 <= 2^22, which covers the five configurations; larger plans report their col_drop.
+// i0 / j0 / k are the outputs of rick_oracle_keys.  perm[r] = input index of the visibility at rank r.
+void rick_oracle_sort_cells(long long M, const int32_t* i0, const int32_t* j0, const int32_t* k, int col_drop,
+                            uint32_t* perm) {
+    std::iota(perm, perm + M, (uint32_t)0);
+    std::stable_sort(perm, perm + M, [=](uint32_t a, uint32_t b) {
+        const bool da = k[a] < 0, db = k[b] < 0;
+        if (da || db) return !da && db;                      // kept before dropped; dropped stay in input order
+        if (k[a] != k[b]) return k[a] < k[b];
+        if (j0[a] / 32 != j0[b] / 32) return j0[a] / 32 < j0[b] / 32;
+        if (i0[a] / 32 != i0[b] / 32) return i0[a] / 32 < i0[b] / 32;
+        if (j0[a] % 32 != j0[b] % 32) return j0[a] % 32 < j0[b] % 32;
+        const int ca = (i0[a] % 32) >> col_drop, cb = (i0[b] % 32) >> col_drop;
+        return ca < cb;
+    });
 }
 
-// D4/D4': the stable order (key, input index).  perm[r] = input index of the visibility at sorted rank r.
+// D4: the stable order (tile key, input index).  perm[r] = input index of the visibility at sorted rank r.
 void rick_oracle_sort(long long M, const uint32_t* key, uint32_t* perm) {
     std::iota(perm, perm + M, (uint32_t)0);
     std::stable_sort(perm, perm + M, [key](uint32_t a, uint32_t b) { return key[a] < key[b]; });

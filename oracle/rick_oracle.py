@@ -45,8 +45,7 @@ def lib():
         L.rick_oracle_keys.argtypes = geo + [C.c_double, C.c_double, C.c_double, C.c_longlong,
                                              f32p, f32p, f32p, f32p, f32p, u32p, i32p, i32p, i32p]
         L.rick_oracle_sort.argtypes = [C.c_longlong, u32p, u32p]
-        L.rick_oracle_sort_key.restype = C.c_int
-        L.rick_oracle_sort_key.argtypes = [C.c_int, C.c_int, C.c_longlong, u32p, i32p, i32p, u32p]
+        L.rick_oracle_sort_cells.argtypes = [C.c_longlong, i32p, i32p, i32p, C.c_int, u32p]
         L.rick_oracle_counting_sort.argtypes = [C.c_longlong, u32p, C.c_uint32, u32p, u64p]
         L.rick_oracle_grid.argtypes = geo + [C.c_double] * 4 + [C.c_longlong, f32p, f32p, f32p, f32p, f32p, f64p]
         L.rick_oracle_plane_transform.argtypes = [C.c_int, f64p]
@@ -134,15 +133,16 @@ def keys(plan: Plan, u, v, w, vis, wt):
     return key, i0, j0, k, int(n)
 
 
-def sort_key(plan: Plan, key: np.ndarray, i0: np.ndarray, j0: np.ndarray) -> Tuple[np.ndarray, int]:
-    """D4': -> (sort_key u32[M], cb): the tile key refined by the top cb bits of the in-tile cell index."""
-    key = np.ascontiguousarray(key, dtype=np.uint32)
+def sort_cells(i0: np.ndarray, j0: np.ndarray, k: np.ndarray, col_drop: int = 0) -> np.ndarray:
+    """D4': stable order by (plane, tile row, tile column, row in tile, column in tile >> col_drop), dropped
+    visibilities (k < 0) last; i0 / j0 / k as returned by keys().  -> perm u32[M] (rank -> input index)."""
     i0 = np.ascontiguousarray(i0, dtype=np.int32)
     j0 = np.ascontiguousarray(j0, dtype=np.int32)
-    out = np.empty(key.shape[0], np.uint32)
-    cb = lib().rick_oracle_sort_key(plan.N, plan.Nw, key.shape[0], _p(key, C.c_uint32), _p(i0, C.c_int32),
-                                    _p(j0, C.c_int32), _p(out, C.c_uint32))
-    return out, int(cb)
+    k = np.ascontiguousarray(k, dtype=np.int32)
+    perm = np.empty(k.shape[0], np.uint32)
+    lib().rick_oracle_sort_cells(k.shape[0], _p(i0, C.c_int32), _p(j0, C.c_int32), _p(k, C.c_int32), int(col_drop),
+                                 _p(perm, C.c_uint32))
+    return perm
 
 
 def sort(key: np.ndarray) -> np.ndarray:

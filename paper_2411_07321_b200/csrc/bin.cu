@@ -18,7 +18,7 @@ namespace {
 constexpr int kRadix = 1 << RICK_RADIX_BITS_MAX;   // 512 digit values at most
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 32;
-constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
+constexpr int kSortTile = kSortThreads * kSortItems;   // 8192 keys per tile
 constexpr int kSortWarps = kSortThreads / 32;
 
 struct SortLayout {
@@ -458,8 +458,7 @@ int rick_bin_init() {
 int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, const float* w, const float2* vis,
                   const float* weight, float* u_s, float* v_s, float* w_s, float2* vis_s, float* weight_s,
                   unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out, void* workspace,
-                  size_t workspace_bytes, long long* n_kept_dev, cudaStream_t st) {
-    (void)workspace_bytes;
+                  long long* n_kept_dev, cudaStream_t st) {
     const RickGeom& g = p->g;
     Workspace ws = carve(workspace, M);
     p->bound = false;

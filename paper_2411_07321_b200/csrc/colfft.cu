@@ -466,7 +466,8 @@ int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int
 int rick_rowfft_impl(rick_plan* p, void* grid, cudaStream_t st) {
     const int N = p->g.N;
     const size_t smem = colfft_smem_bytes(N) + 2 * (size_t)(N * kC / 512) * kRowPad * sizeof(float2);
-    static bool attr_done = false;
+    static bool attr_done_dev[RICK_MAX_DEVICES] = {};      // the opt-in is per device
+    bool& attr_done = attr_done_dev[p->device & (RICK_MAX_DEVICES - 1)];
     if (!attr_done) {
         const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
         if (cudaFuncSetAttribute(k_rowfft<8>, a, (int)(colfft_smem_bytes(256) + 2 * (256 * kC / 512) * kRowPad * sizeof(float2))) != cudaSuccess ||

@@ -459,11 +459,12 @@ int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
     constexpr int L = 16;                                   // records per thread and stage
     constexpr int NBUF = 2;                                 // double-buffered stages (1 was measured: no gain)
     constexpr int smem = NBUF * 3 * kRunThreads * (L / 2) * 16;   // NBUF buffers of three streams, 48 KB each
-    static bool attr_done = false;
-    if (!attr_done) {
+    static bool attr_done[RICK_MAX_DEVICES] = {};      // the opt-in is per device
+    const int dv = p->device & (RICK_MAX_DEVICES - 1);
+    if (!attr_done[dv]) {
         if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return RICK_ECUDA;
-        attr_done = true;
+        attr_done[dv] = true;
     }
     TapConst tc;
     for (int t = 0; t < 8; ++t) {

@@ -1,4 +1,5 @@
 // plan.cu -- plan lifetime, cuFFT stage, stage timers, host<->device entry points of librick_b200.
+#include <cmath>
 #include <math.h>
 #include <new>
 #include <stdlib.h>
@@ -97,26 +98,22 @@ int build_fft(rick_plan* p) {
 }
 
 
-// modified Bessel functions by their power series (all terms positive)
-double bessel_i0_series(double x) {
-    const double q = 0.25 * x * x;
-    double term = 1.0, sum = 1.0;
-    for (int k = 1; k < 500; ++k) {
-        term *= q / ((double)k * (double)k);
-        sum += term;
-        if (term < 1e-17 * sum) break;
-    }
-    return sum;
+// Modified Bessel functions of the first kind through the C++17 special-function library (libstdc++'s
+// std::cyl_bessel_i: series for small arguments, asymptotic / uniform expansions beyond).
+double bessel_i0_lib(double x) { return std::cyl_bessel_i(0.0, fabs(x)); }
+double bessel_i1_over_x_lib(double x) {        // I1(x) / x -> 1/2 at 0
+    const double ax = fabs(x);
+    if (ax < 1e-8) return 0.5;
+    return std::cyl_bessel_i(1.0, ax) / ax;
 }
-double bessel_i1_over_x_series(double x) {     // I1(x) / x = sum_k (x^2/4)^k / (k! (k+1)!) / 2
-    const double q = 0.25 * x * x;
-    double term = 0.5, sum = 0.5;
-    for (int k = 1; k < 500; ++k) {
-        term *= q / ((double)k * (double)(k + 1));
-        sum += term;
-        if (term < 1e-17 * sum) break;
-    }
-    return sum;
+
+// sinh(sqrt t) / sqrt t as one entire function of t (it continues to sin(sqrt -t) / sqrt -t for t < 0):
+// the transform of the Kaiser-Bessel window is 2 a_t sinhc(beta^2 - (2 pi a_t nu)^2) / I0(beta) on both
+// sides of the edge of the main lobe [D8-KB]
+double sinhc_of_square(double t) {
+    if (fabs(t) < 1e-3) return 1.0 + (t / 6.0) * (1.0 + (t / 20.0) * (1.0 + t / 42.0));
+    const double r = sqrt(fabs(t));
+    return t > 0.0 ? sinh(r) / r : sin(r) / r;
 }
 
 // D8 / D8-KB: 1 / t[p] on the device.  Gaussian: t[p] = c0 exp(-2 pi^2 sigma^2 nu_p^2),
@@ -130,15 +127,10 @@ int upload_taper(rick_plan* p) {
     const double pi = 3.14159265358979323846;
     const double a_t = (double)g.h + 0.5;
     if (g.kernel == RICK_KERNEL_KB) {
-        const double i0b = bessel_i0_series(p->kb_beta);
+        const double scale = bessel_i0_lib(p->kb_beta) / (2.0 * a_t), b2 = p->kb_beta * p->kb_beta;
         for (int i = 0; i < N; ++i) {
-            const double nu = (double)(i - N / 2) / (double)N;
-            const double y = 2.0 * pi * a_t * nu;
-            const double z2 = p->kb_beta * p->kb_beta - y * y;
-            double sc = 1.0;
-            if (z2 > 1e-24) { const double z = sqrt(z2); sc = sinh(z) / z; }
-            else if (z2 < -1e-24) { const double z = sqrt(-z2); sc = sin(z) / z; }
-            inv_t[i] = i0b / (2.0 * a_t * sc);
+            const double y = 2.0 * pi * a_t * ((double)(i - N / 2) / (double)N);
+            inv_t[i] = scale / sinhc_of_square(b2 - y * y);
         }
     } else {
         const double sigma = g.sigma;
@@ -161,10 +153,10 @@ int upload_taper(rick_plan* p) {
 // Chebyshev nodes of [-1, 1]; returns the largest error of the fp32-rounded polynomials over a fine sample.
 double fit_kb_polynomials(rick_plan* p) {
     const int T = RICK_KB_POLY_TERMS, S = p->g.S, h = p->g.h;
-    const double a_t = (double)h + 0.5, beta = p->kb_beta, i0b = bessel_i0_series(beta), pi = 3.14159265358979323846;
+    const double a_t = (double)h + 0.5, beta = p->kb_beta, i0b = bessel_i0_lib(beta), pi = 3.14159265358979323846;
     auto win = [&](double d) {
         const double r = d / a_t, arg = 1.0 - r * r;
-        return bessel_i0_series(beta * sqrt(arg > 0.0 ? arg : 0.0)) / i0b;
+        return bessel_i0_lib(beta * sqrt(arg > 0.0 ? arg : 0.0)) / i0b;
     };
     double worst = 0.0;
     for (int a = 0; a < S; ++a) {
@@ -197,6 +189,20 @@ double fit_kb_polynomials(rick_plan* p) {
     return worst;
 }
 
+// copy stream and hand-over events of rick_image_from_host_chunked, created with the plan
+int pipe_init(rick_plan* p) {
+    if (p->pipe_ready) return RICK_OK;
+    RICK_CUDA(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming));
+        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
+    }
+    RICK_CUDA(cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
+    for (int i = 0; i < RICK_IMAGE_PARTS; ++i) RICK_CUDA(cudaEventCreateWithFlags(&p->ev_part[i], cudaEventDisableTiming));
+    p->pipe_ready = true;
+    return RICK_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -208,7 +214,9 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     if (N < 32 || N > 32768 || (N % RICK_TILE) != 0) return RICK_EINVAL;
     if (Nw < 1 || Nw > 4096) return RICK_EINVAL;
     if (support < 3 || support > 15 || (support % 2) == 0) return RICK_EINVAL;
-    if (!(sigma > 0.0) || !isfinite(sigma)) return RICK_EINVAL;
+    // sigma >= 1/4 cell: below that the tap recurrence g(d0 + s) = g(d0) E^s g(s) overflows E^s while g(s)
+    // underflows (inf * 0), and a Gaussian that narrow is not a usable gridding kernel anyway
+    if (!(sigma >= 0.25) || !isfinite(sigma)) return RICK_EINVAL;
     if (!isfinite(w_min) || !isfinite(w_max) || !(w_max > w_min)) return RICK_EINVAL;
     if (!(dl > 0.0) || !isfinite(dl) || !((double)N * dl < 1.4142135623730951)) return RICK_EINVAL;
     const long long T = N / RICK_TILE;
@@ -257,6 +265,7 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { delete p; return RICK_ECUDA; }
     p->sm_count = sms > 0 ? sms : 148;
+    p->device = dev;
 
     {
         const int rc = upload_taper(p);
@@ -267,6 +276,10 @@ int rick_plan_create(int N, int Nw, int support, double sigma, double w_min, dou
             rick_plan_destroy(p);
             return RICK_ECUDA;
         }
+    }
+    if (pipe_init(p) != RICK_OK) {
+        rick_plan_destroy(p);
+        return RICK_ECUDA;
     }
     *out = p;
     return RICK_OK;
@@ -288,7 +301,7 @@ int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
     if (kind == RICK_KERNEL_KB) {
         p->kb_beta = param;
         const int nL = 8192;
-        const double a_t = (double)g.h + 0.5, hstep = a_t / nL, i0b = bessel_i0_series(param);
+        const double a_t = (double)g.h + 0.5, hstep = a_t / nL, i0b = bessel_i0_lib(param);
         float2* lf = (float2*)malloc(sizeof(float2) * (nL + 1));
         double2* ld = (double2*)malloc(sizeof(double2) * (nL + 1));
         double* gv = (double*)malloc(sizeof(double) * (nL + 1));
@@ -296,9 +309,9 @@ int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
         for (int i = 0; i <= nL; ++i) {
             const double d = i * hstep, r = d / a_t;
             const double arg = 1.0 - r * r, z = param * sqrt(arg > 0.0 ? arg : 0.0);
-            gv[i] = bessel_i0_series(z) / i0b;
+            gv[i] = bessel_i0_lib(z) / i0b;
             // g'(d) = -(beta^2 d / a_t^2) (I1(z) / z) / I0(beta)
-            ld[i] = make_double2(gv[i], hstep * (-(param * param) * d / (a_t * a_t) * bessel_i1_over_x_series(z) / i0b));
+            ld[i] = make_double2(gv[i], hstep * (-(param * param) * d / (a_t * a_t) * bessel_i1_over_x_lib(z) / i0b));
         }
         for (int i = 0; i <= nL; ++i) lf[i] = make_float2((float)gv[i], i < nL ? (float)(gv[i + 1] - gv[i]) : 0.f);
         cudaError_t e = cudaSuccess;
@@ -406,7 +419,7 @@ int rick_bin(rick_plan* p, long long M, const float* u, const float* v, const fl
     cudaStream_t st = (cudaStream_t)stream;
     StageTimer tm(p, RICK_T_BIN, st);
     return rick_bin_impl(p, M, u, v, w, (const float2*)vis, weight, u_s, v_s, w_s, (float2*)vis_s, weight_s,
-                         key_out, perm_out, bin_start_out, workspace, workspace_bytes, n_kept_dev, st);
+                         key_out, perm_out, bin_start_out, workspace, n_kept_dev, st);
 }
 
 int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
@@ -507,19 +520,6 @@ int rick_image_from_host(rick_plan* p, long long M, const float* u_h, const floa
     return RICK_OK;
 }
 
-static int pipe_init(rick_plan* p) {
-    if (p->pipe_ready) return RICK_OK;
-    RICK_CUDA(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
-    for (int b = 0; b < 2; ++b) {
-        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming));
-        RICK_CUDA(cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
-    }
-    RICK_CUDA(cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
-    for (int i = 0; i < RICK_IMAGE_PARTS; ++i) RICK_CUDA(cudaEventCreateWithFlags(&p->ev_part[i], cudaEventDisableTiming));
-    p->pipe_ready = true;
-    return RICK_OK;
-}
-
 int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, const float* v_h,
                                  const float* w_h, const void* vis_h, const float* weight_h,
                                  const rick_device_buffers* d, int n_chunks, double* image_host,
@@ -528,8 +528,7 @@ int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, co
     if (n_chunks < 2 || M < 2 * 1024)
         return rick_image_from_host(p, M, u_h, v_h, w_h, vis_h, weight_h, d, image_host, stream);
     if (!u_h || !v_h || !w_h || !vis_h || !weight_h) return RICK_EINVAL;
-    int rc = pipe_init(p);
-    if (rc != RICK_OK) return rc;
+    int rc = RICK_OK;
     cudaStream_t st = (cudaStream_t)stream, cs = p->copy_stream;
     // chunk length: a multiple of 1024 visibilities, two of them within the staging capacity M
     long long c = (M + n_chunks - 1) / n_chunks;

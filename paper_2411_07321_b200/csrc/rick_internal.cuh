@@ -89,7 +89,10 @@ struct rick_plan {
     bool ev_valid[RICK_T_COUNT];
     long long launches;
     int sm_count;
+    int device;              // CUDA device the plan was created on (kernel attributes are set per device)
 };
+
+#define RICK_MAX_DEVICES 64
 
 #define RICK_CUDA(call)                                  \
     do {                                                 \
@@ -99,7 +102,7 @@ struct rick_plan {
 
 #define RICK_LAUNCH_CHECK()                              \
     do {                                                 \
-        if (cudaPeekAtLastError() != cudaSuccess) {      \
+        if (cudaGetLastError() != cudaSuccess) {         \
             return RICK_ECUDA;                           \
         }                                                \
     } while (0)
@@ -154,8 +157,7 @@ void rick_stage_end(rick_plan* p, int stage, cudaStream_t st);
 int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, const float* w,
                   const float2* vis, const float* weight, float* u_s, float* v_s, float* w_s,
                   float2* vis_s, float* weight_s, unsigned* key_out, unsigned* perm_out,
-                  unsigned long long* bin_start_out, void* workspace, size_t workspace_bytes,
-                  long long* n_kept_dev, cudaStream_t st);
+                  unsigned long long* bin_start_out, void* workspace, long long* n_kept_dev, cudaStream_t st);
 size_t rick_bin_workspace_bytes(const rick_plan* p, long long M);
 int rick_bin_init();   // one-time kernel attributes (dynamic shared memory opt-in)
 int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st);

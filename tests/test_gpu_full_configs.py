@@ -56,8 +56,8 @@ def test_full_config(name):
     one = np.ones(n_kept, np.complex64)
     skey, si0, sj0, _, sn = O.keys(O.Plan(**pa), su, sv, sw, one, np.ones(n_kept, np.float32))
     assert sn == n_kept
-    ssk, _ = O.sort_key(O.Plan(**pa), skey, si0, sj0)
-    assert np.all(np.diff(ssk.astype(np.int64)) >= 0)
+    ssk = (skey.astype(np.int64) * 32 + (sj0 & 31)) * 32 + (si0 & 31)      # D4' order: (plane, tile, row, column)
+    assert np.all(np.diff(ssk) >= 0)
     del su, sv, sw, one, skey, si0, sj0, ssk, okey, oi0, oj0, ok, kept
     ref, n2, st = O.image(O.Plan(**pa), *hv, return_timing=True)
     assert n2 == n_kept

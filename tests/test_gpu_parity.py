@@ -48,11 +48,11 @@ def check_bin(im, vis, pa):
     u, v, w, vv, wt = vis.numpy()
     plan = O.Plan(**pa)
     key, perm, bs, n_kept = run_bin(im, vis)
-    okey, oi0, oj0, _, on = O.keys(plan, u, v, w, vv, wt)
+    okey, oi0, oj0, ok, on = O.keys(plan, u, v, w, vv, wt)
     assert np.array_equal(key, okey)
     assert n_kept == on
-    osk, _ = O.sort_key(plan, okey, oi0, oj0)      # D4': the key rick_bin sorts by
-    operm = O.sort(osk)
+    _, _, cell_bits = B.rick_plan_sort_layout(im.plan)
+    operm = O.sort_cells(oi0, oj0, ok, col_drop=10 - cell_bits)   # D4' (10 cell bits: the exact cell)
     assert np.array_equal(perm, operm)
     _, obs = O.counting_sort(okey, plan.n_bins)
     assert np.array_equal(bs, obs)

@@ -125,44 +125,59 @@ def test_stable_sort_three_ways():
     assert key[perm[-1]] == n_bins    # the sentinel sorts last
 
 
-def test_sort_key_refines_tile_key():
-    """D4': hand values, the refinement property (same grouping by tile, cells adjacent inside a tile)
-    and the sentinel, for plans where all 10 cell bits fit (Nw T^2 = 2^22 fills the 32 bits exactly),
-    one that keeps 9 bits (2^23) and one that keeps 6 (2^26)."""
-    # hand case: N=256 (T=8), Nw=8 -> n_bins=512, cb=10; vis at i0=131, j0=37, k=3:
-    # key=(3*8+1)*8+4=204, cell=(37&31)*32+(131&31)=5*32+3=163 -> 204*1024+163
-    plan = O.Plan(N=256, Nw=8, support=7, sigma=1.0, w_min=0.0, w_max=8.0, dl=0.2 / 256)
-    key = np.array([204, 512, 0], np.uint32)
-    sk, cb = O.sort_key(plan, key, np.array([131, -1, 3], np.int32), np.array([37, -1, 3], np.int32))
-    assert cb == 10 and list(sk) == [204 * 1024 + 163, 512 * 1024 - 1, 3 * 32 + 3]
+def test_sort_cells_hand_case():
+    """D4' order written out by hand: N = 64 (2 x 2 tiles), visibilities given by (i0, j0, k); k < 0 = dropped.
+    Expected: plane first, then tile row, tile column, row in tile, column in tile, then input index."""
+    #            idx: 0   1   2   3   4   5   6   7   8
+    i0 = np.array([40,  5,  5, 33,  5, -1,  6,  5, 40], np.int32)
+    j0 = np.array([ 3,  3, 35,  3,  3, -1,  3,  2,  3], np.int32)
+    k = np.array([ 0,  1,  0,  0,  0, -1,  0,  0,  0], np.int32)
+    # plane 0: tile (row 0, col 0): (j0 2, i0 5) idx 7; (3, 5) idx 4; (3, 6) idx 6
+    #          tile (row 0, col 1): (3, 33) idx 3; (3, 40) idx 0, 8 (input order)
+    #          tile (row 1, col 0): (35, 5) idx 2
+    # plane 1: idx 1; dropped: idx 5
+    assert list(O.sort_cells(i0, j0, k)) == [7, 4, 6, 3, 0, 8, 2, 1, 5]
+    # col_drop = 1: columns 4|5 and 6|7 merge: (3,5) idx 4 and (3,6) idx 6 stay apart, (3,4)/(3,5) would merge
+    i0b = np.array([5, 4, 7, 6], np.int32)
+    z = np.zeros(4, np.int32)
+    assert list(O.sort_cells(i0b, z + 3, z, col_drop=1)) == [0, 1, 2, 3]      # {5,4} tie -> input order, then {7,6}
+    assert list(O.sort_cells(i0b, z + 3, z, col_drop=0)) == [1, 0, 3, 2]
+
+
+def test_sort_cells_properties():
+    """D4' on random inputs: a refinement of the D4 order (sorted by (plane, tile) key), lexicographic inside a
+    tile, equal nearest cells contiguous and in input order, dropped visibilities last in input order; and
+    the same permutation as numpy's lexsort over the same tuple."""
     rng = np.random.default_rng(3)
-    for N, Nw, ecb in ((512, 16, 10), (16384, 16, 10), (16384, 32, 9), (32768, 64, 6)):
+    for N, Nw in ((512, 16), (2048, 4)):
         plan = O.Plan(N=N, Nw=Nw, support=9, sigma=1.3, w_min=-50.0, w_max=50.0, dl=0.5 / N)
         M = 30000
         du = 1.0 / (N * plan.dl)
         u = rng.uniform(-0.52 * N * du, 0.52 * N * du, M).astype(np.float32)
         v = rng.uniform(-0.52 * N * du, 0.52 * N * du, M).astype(np.float32)
-        u[:2000] = rng.uniform(40 * du, 60 * du, 2000).astype(np.float32)    # a dense patch: real runs
-        v[:2000] = rng.uniform(40 * du, 60 * du, 2000).astype(np.float32)
-        u[-1], v[-1] = (N // 2 - 1 - 4) * du, (N // 2 - 1 - 4) * du         # the last cell D5 keeps
+        u[:4000] = rng.uniform(40 * du, 60 * du, 4000).astype(np.float32)    # a dense patch: real runs
+        v[:4000] = rng.uniform(40 * du, 60 * du, 4000).astype(np.float32)
         w = rng.uniform(-55, 55, M).astype(np.float32)
-        w[-1] = 50.0
         key, i0, j0, k, n_kept = O.keys(plan, u, v, w, np.ones(M, np.complex64), np.ones(M, np.float32))
-        sk, cb = O.sort_key(plan, key, i0, j0)
-        assert cb == ecb
-        kept = key < plan.n_bins
-        assert kept[-1] and 0 < n_kept < M
-        assert np.all(sk[~kept] == (plan.n_bins << cb) - 1) and np.all(sk[kept].astype(np.int64) < sk[~kept][0])
-        assert np.array_equal(sk[kept] >> cb, key[kept])                      # refinement of the tile key
-        cell = ((j0[kept] & 31) << 5) | (i0[kept] & 31)
-        assert np.array_equal(sk[kept] & ((1 << cb) - 1), cell >> (10 - cb))
-        perm = O.sort(sk)
-        assert np.all(np.diff(key[perm].astype(np.int64)) >= 0)              # still sorted by (plane, tile)
-        if cb == 10:   # equal sort keys <=> equal nearest cell and plane
-            full = (k[kept].astype(np.int64) * N + j0[kept]) * N + i0[kept]
-            _, inv_a = np.unique(full, return_inverse=True)
-            _, inv_b = np.unique(sk[kept], return_inverse=True)
-            assert len(set(zip(inv_a.tolist(), inv_b.tolist()))) == inv_a.max() + 1 == inv_b.max() + 1
+        perm = O.sort_cells(i0, j0, k).astype(np.int64)
+        assert sorted(perm.tolist()) == list(range(M)) and 0 < n_kept < M
+        kept, drop = perm[:n_kept], perm[n_kept:]
+        assert np.all(k[kept] >= 0) and np.all(k[drop] < 0) and np.all(np.diff(drop) > 0)
+        assert np.all(np.diff(key[perm].astype(np.int64)) >= 0)              # still sorted by the D4 tile key
+        cell = (j0[kept].astype(np.int64) & 31) * 32 + (i0[kept] & 31)
+        same_tile = np.diff(key[kept].astype(np.int64)) == 0
+        assert np.all(np.diff(cell)[same_tile] >= 0)                          # lexicographic (row, column) in a tile
+        full = (k[kept].astype(np.int64) * N + j0[kept]) * N + i0[kept]
+        same_cell = np.diff(full) == 0
+        assert np.all(np.diff(kept)[same_cell] > 0)                           # stable
+        assert len(np.unique(full)) == 1 + int((~same_cell).sum())            # equal cells are contiguous
+        big = np.where(k < 0, 1 << 40, 0).astype(np.int64)
+        ref = np.lexsort((np.arange(M), i0 & 31, j0 & 31, i0 >> 5, j0 >> 5, k.astype(np.int64) + big))
+        assert np.array_equal(perm, ref)
+        # col_drop = 2: columns are compared in groups of four
+        perm2 = O.sort_cells(i0, j0, k, col_drop=2).astype(np.int64)
+        ref2 = np.lexsort((np.arange(M), (i0 & 31) >> 2, j0 & 31, i0 >> 5, j0 >> 5, k.astype(np.int64) + big))
+        assert np.array_equal(perm2, ref2)
 
 
 # ------------------------------------------------------------------------------------------------
