@@ -3,9 +3,10 @@
 
 A step = one pass of the whole hot path (rick_bin -> rick_grid (zero + grid) -> rick_fft_planes ->
 rick_wcorrect_accumulate) over one batch of seeded synthetic visibilities already resident in HBM.
-Workload at N=1: BASELINE.json configs[1] ("10M": 1e7 visibilities, 2048^2 x 32 planes, complex64 mesh).
+Workload at N=1: BASELINE.json configs[4] ("hotspot": 1e9 visibilities, 16384^2 x 16 planes, complex64 mesh,
+support 9), the largest configuration that fits one GPU; the other four by --config.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 10M] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config hotspot] [--impl reference]
 
 N > 1 (torchrun): the path does not shard ("replicas only"): every rank images its own copy
 of the workload on its own GPU, no data-path collective; value = visibilities of all ranks / max time.
@@ -39,13 +40,13 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def _traffic(kernel: str, workload: str = "10M"):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary (captured on the
-    workload the file names), or None."""
+def _traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full
+    summary captured on `workload` (profiles/traffic.json: {workload: {kernel: bytes}}), or None when there is
+    no capture of this kernel on this workload."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            d = json.load(f)
-            return d.get(kernel) if d.get("_workload", "10M") == workload else None
+            return json.load(f).get(workload, {}).get(kernel)
     except Exception:
         return None
 
@@ -121,29 +122,33 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def _oracle_sample(cfg, vis_host, pa, sample_M: int):
-    """Time the oracle, as it stands, on the first `sample_M` visibilities with the full plan (all Nw planes
-    are gridded, transformed and w-corrected).  Returns (seconds per stage, n_kept of the sample, threads)."""
+def _one_plane(pa, vis_host, sample_M: int):
+    """The bounded oracle sample: the first `sample_M` visibilities imaged through ONE w-plane of the
+    configuration's mesh (same N, support, sigma, dl; the plan's whole w range mapped to a single plane), by
+    the oracle's own whole-path call as it stands.  Its per-visibility stages (keys, gridding) scale with M,
+    its per-plane stages (FFT, w-correction) with the plane count.  -> (stage seconds, n_kept, wall s, threads)"""
     from oracle import rick_oracle as O
     u, v, w, vv, wt = (a[:sample_M] for a in vis_host)
+    pa1 = dict(pa, Nw=1)
     t0 = time.perf_counter()
-    _, n_kept, st = O.image(O.Plan(**pa), u, v, w, vv, wt, return_timing=True)
+    _, n_kept, st = O.image(O.Plan(**pa1), u, v, w, vv, wt, return_timing=True)
     total = time.perf_counter() - t0
     return st, n_kept, total, O.threads()
 
 
-def cpu_baseline(cfg, vis_host, pa, M: int):
-    """The oracle timed on a bounded sample; the whole-workload time is per-visibility stages scaled by
-    M / M_sample plus the per-plane stages (FFT, w-correction), which do not depend on M."""
-    sample_M = min(M, 1_000_000)
-    st, n_kept_s, total, threads = _oracle_sample(cfg, vis_host, pa, sample_M)
+def cpu_baseline(cfg, vis_host, pa, M: int, n_kept: int, sample_M: int = 1_000_000):
+    """The oracle timed on a bounded sample (see _one_plane); the whole-workload time is estimated as
+    per-visibility stages x M / M_sample + per-plane stages x Nw.  Same numerator as the GPU line (kept
+    visibilities)."""
+    sample_M = min(M, sample_M)
+    st, n_kept_s, total, threads = _one_plane(pa, vis_host, sample_M)
     scale = M / sample_M
-    est = (st["keys"] + st["grid"]) * scale + st["fft"] + st["wcorrect"]
+    est = (st["keys"] + st["grid"]) * scale + (st["fft"] + st["wcorrect"]) * pa["Nw"]
     return {
-        "value": M / est, "unit": UNIT, "cores": threads, "kind": "oracle",
-        "sample": (f"first {sample_M} of {M} visibilities through the full plan ({pa['N']}^2 x {pa['Nw']} planes): "
+        "value": n_kept / est, "unit": UNIT, "cores": threads, "kind": "oracle",
+        "sample": (f"first {sample_M} of {M} visibilities through one of the {pa['Nw']} planes of the {pa['N']}^2 mesh: "
                    f"keys+grid {st['keys'] + st['grid']:.2f} s scaled x{scale:.1f}, fft {st['fft']:.2f} s and "
-                   f"w-correct {st['wcorrect']:.2f} s taken as measured; sample wall {total:.2f} s"),
+                   f"w-correct {st['wcorrect']:.2f} s per plane scaled x{pa['Nw']}; sample wall {total:.2f} s"),
         "stage_seconds_sample": {k: round(float(x), 4) for k, x in st.items()},
         "est_seconds_full": est,
     }
@@ -165,21 +170,22 @@ def run_reference(args):
     times = []
     last = None
     for i in range(args.warmup + args.steps):
-        st, n_kept, total, threads = _oracle_sample(scfg, host, pa, sample_M)
+        st, n_kept, total, threads = _one_plane(pa, host, sample_M)
         if i >= args.warmup:
             times.append(total)
         last = (st, n_kept, threads)
     sec = sum(times) / len(times)
-    value = sample_M / sec
     st, n_kept, threads = last
+    value = n_kept / sec
+    sample = (f"each step images the first {sample_M} visibilities of the workload ({n_kept} kept) through ONE w-plane "
+              f"of the {pa['N']}^2 mesh (the oracle's per-plane FFT and w-correction cost {st['fft'] + st['wcorrect']:.1f} s "
+              f"per plane at this size; all {pa['Nw']} planes per step would not end within minutes)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.config, "N": pa["N"], "Nw": pa["Nw"], "support": pa["support"],
-                   "sample": f"each step images the first {sample_M} visibilities of the workload with the full plan"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
-                         "sample": f"first {sample_M} of {cfg.M} visibilities, all {pa['Nw']} planes, per step"},
+        "config": {"workload": args.config, "N": pa["N"], "Nw": pa["Nw"], "support": pa["support"], "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
@@ -188,18 +194,19 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="10M")
+    ap.add_argument("--config", default="hotspot", choices=["tiny", "10M", "100M", "500M", "hotspot"],
+                    help="BASELINE.json workload; default: the largest single-GPU configuration")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--ref-sample", type=int, default=1_000_000)
+    ap.add_argument("--ref-sample", type=int, default=200_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fusion", action="store_true", help="2-D cuFFT + separate w-correction kernel")
     ap.add_argument("--fusion", type=int, default=2, choices=[1, 2],
-                    help="rick_plan_set_fusion mode where the plan supports it: 1 fused column transform, 2 + row occupancy")
+                    help="rick_plan_set_fusion mode: 1 fused column transform, 2 + row occupancy")
     ap.add_argument("--kernel", default="gauss", choices=["gauss", "kb"],
                     help="gridding kernel: the Gaussian of BASELINE.json (default) or the paper's Kaiser-Bessel (beta = 2.34 S)")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-chunks", type=int, default=4,
                     help="time slices of rick_image_from_host_chunked in the e2e region (1: one copy, then compute)")
     args = ap.parse_args()
@@ -232,6 +239,7 @@ def main():
     im = B.Imager(dtype=cfg.dtype, M_max=M, fused=0 if args.no_fusion else args.fusion, kernel=args.kernel, beta=2.34 * cfg.support, **pa)
     cell = 16 if cfg.dtype == "c128" else 8
     mesh_bytes = cfg.Nw * cfg.N * cfg.N * cell
+    fma_tflops, add_tinst = B.rick_measure_fp32_rate()
 
     def step():
         im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight)
@@ -261,7 +269,7 @@ def main():
     if dist is not None:
         dist.barrier()
     ms_per_step = ms / args.steps
-    value = job_value(M, world, ms_per_step)
+    value = job_value(n_kept, world, ms_per_step)            # gridded (kept) visibilities per second, SURVEY 8(d)
 
     # per-stage CUDA-event times (events recorded by the library on the launch stream), same workload
     per = {k: [] for k in B.RICK_T_NAMES}
@@ -278,35 +286,50 @@ def main():
     rows_total = cfg.Nw * cfg.N
     rows_defined = B.rick_plan_rows_defined(im.plan) if im.fused == 2 else rows_total
     live_bytes = mesh_bytes * rows_defined // rows_total
-    alg = {   # algorithmic bytes per launch
+    one_sweep = bool(im.fused) and cfg.dtype == "c64" and cfg.N <= 2048      # colfft.cu; else the split engine (colsplit.cu)
+    split = bool(im.fused) and not one_sweep
+    if not im.fused:
+        fft_rows_b, col_a_b, fft_b, wc_b = 0, 0, 4 * mesh_bytes, mesh_bytes + cfg.N * cfg.N * 8
+    elif one_sweep:
+        fft_rows_b = 2 * live_bytes          # mode 2: own row kernel on the defined rows; mode 1: live = mesh
+        col_a_b, fft_b, wc_b = 0, fft_rows_b, live_bytes + cfg.N * cfg.N * 8
+    else:
+        fft_rows_b = 2 * mesh_bytes          # batched library row transforms of every row
+        col_a_b = live_bytes + mesh_bytes    # sweep A reads the defined rows, writes every row
+        fft_b, wc_b = fft_rows_b + col_a_b, mesh_bytes + cfg.N * cfg.N * 8
+    alg = {   # algorithmic bytes per stage
         "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
         # sort: first pass 4 r + 8 w, middle passes 8 r + 8 w, last pass 8 r and, fused into it, the gather
         # (one 32-B record in, sorted SoA 24 B + gridder records 24 B out per kept visibility)
         "sort": ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept,
-        "gather": 0,                                 # rides in the last sort pass (rick_bin without perm_out)
-        "zero": live_bytes,
+        "zero": live_bytes if im.fused == 2 else mesh_bytes,
         "grid": 24 * n_kept,
-        "fft": (2 if im.fused else 4) * live_bytes,      # fused: row transforms only (one read + write)
-        "wcorrect": live_bytes + cfg.N * cfg.N * 8,      # fused: column transforms + screen + sum, one read
+        "fft": fft_b, "fft_rows": fft_rows_b, "fft_col_a": col_a_b,
+        "wcorrect": wc_b,
     }
     stages = {}
     for k, b in alg.items():
-        if k == "gather":
-            continue
         t = stage_ms[k]
-        stages[k] = {"ms": round(t, 4), "alg_bytes": b, "gbs": (b / (t * 1e-3) / 1e9) if t > 0 else None,
-                     "frac": (b / (t * 1e-3) / 1e9 / peak) if t > 0 else None}
+        if b == 0 or t <= 0:
+            continue
+        stages[k] = {"ms": round(t, 4), "alg_bytes": b, "gbs": b / (t * 1e-3) / 1e9, "frac": b / (t * 1e-3) / 1e9 / peak}
     zg = stage_ms["zero"] + stage_ms["grid"]
     stages["zero+grid"] = {"ms": round(zg, 4), "alg_bytes": alg["zero"] + alg["grid"],
                            "gbs": (alg["zero"] + alg["grid"]) / (zg * 1e-3) / 1e9,
                            "frac": (alg["zero"] + alg["grid"]) / (zg * 1e-3) / 1e9 / peak,
                            "vis_per_s": n_kept / (zg * 1e-3),
                            "frac_dense_mesh_definition": (mesh_bytes + alg["grid"]) / (zg * 1e-3) / 1e9 / peak}
+    binzg = stage_ms["bin"] + zg
+    stages["bin+zero+grid"] = {"ms": round(binzg, 4), "vis_per_s": n_kept / (binzg * 1e-3)}
     # the dominant kernel = the library kernel with the largest total time in a step; its roofline numbers
-    # are per launch (sort: n_pass launches of k_onesweep, the average pass)
-    kernels = {"grid": ("k_grid_rec" if cfg.dtype == "c64" else "k_grid_runs", 1),
-               "wcorrect": ("k_colfft_wcorrect" if im.fused else "k_wcorrect", 1), "keygen": ("k_keygen", 1),
-               "sort": ("k_onesweep", n_pass)}
+    # are per launch (sort: n_pass launches of k_onesweep, the average pass), against the measured HBM copy rate
+    kernels = {"grid": ("k_grid_rec" if cfg.dtype == "c64" else "k_grid_runs", 1), "keygen": ("k_keygen", 1),
+               "sort": ("k_onesweep", n_pass),
+               "wcorrect": ("k_col_b" if split else ("k_colfft_wcorrect" if one_sweep else "k_wcorrect"), 1)}
+    if split:
+        kernels["fft_col_a"] = ("k_col_a", 1)
+    elif one_sweep and im.fused == 2:
+        kernels["fft_rows"] = ("k_rowfft", 1)
     dom = max(kernels, key=lambda k: stage_ms[k])
     kname, n_launch = kernels[dom]
     launch_ms = stage_ms[dom] / n_launch
@@ -315,29 +338,33 @@ def main():
     roofline = {"bound": "hbm", "kernel": kname, "stage": dom, "launches_per_step": n_launch,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": _traffic(kname, args.config), "peak_source": peak_src,
-                "launch_ms": launch_ms, "alg_bytes_per_launch": launch_bytes}
-    if kname == "k_colfft_wcorrect":
-        # the fused column transform is bound by fp32 instruction issue, not by HBM (profiles/): report it against
-        # the fp32 ALU peak DESIGN.md section 5 derives (148 SMs x 128 lanes x 2 flop x 1.965 GHz), with the
-        # 5 N log2 N flop of every column transform; the HBM view stays beside it
-        import math
-        flops = 5.0 * cfg.N * math.log2(cfg.N) * cfg.N * cfg.Nw
-        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        roofline = {"bound": "alu", "kernel": kname, "stage": dom, "launches_per_step": n_launch,
-                    "achieved": flops / (launch_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
-                    "frac": flops / (launch_ms * 1e-3) / 1e12 / alu_peak,
-                    "traffic": _traffic(kname + ("_mode2" if im.fused == 2 else ""), args.config),
-                    "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 (FMA) x 1.965 GHz (DESIGN.md section 5)",
-                    "launch_ms": launch_ms, "alg_flops_per_launch": flops,
-                    "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                            "alg_bytes_per_launch": launch_bytes}}
+                "launch_ms": launch_ms, "alg_bytes_per_launch": launch_bytes,
+                "share_of_step": stage_ms[dom] / ms_per_step}
+    # instruction-issue view of the transform kernels against the fp32 rates measured in this run
+    # (rick_measure_fp32_rate: a register-resident FMA / ADD chain on every SM), 5 L log2 L flop per L-point transform
+    import math
+    alu = {"fp32_fma_tflops_measured": fma_tflops, "fp32_add_tinst_measured": add_tinst}
+    if cfg.dtype == "c64" and im.fused:
+        n_el = cfg.N * cfg.N * cfg.Nw
+        if one_sweep:
+            alu["k_colfft_wcorrect_tflops"] = 5.0 * math.log2(cfg.N) * n_el / (stage_ms["wcorrect"] * 1e-3) / 1e12
+        else:
+            n2 = 1 << ((int(math.log2(cfg.N)) + 1) // 2)
+            alu["k_col_a_tflops"] = 5.0 * math.log2(cfg.N // n2) * n_el / (stage_ms["fft_col_a"] * 1e-3) / 1e12
+            alu["k_col_b_tflops"] = 5.0 * math.log2(n2) * n_el / (stage_ms["wcorrect"] * 1e-3) / 1e12
+    roofline["alu_view"] = alu
 
-    # end to end through rick_image_from_host: pinned host inputs -> host image, copies inside the region
-    host = [x.cpu() for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
+    # end to end through rick_image_from_host(_chunked): pinned host inputs -> host image, copies inside the region
+    host = [torch.empty(x.shape, dtype=x.dtype, pin_memory=args.e2e_steps > 0) for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]
+    for h, x in zip(host, (vis.u, vis.v, vis.w, vis.vis, vis.weight)):
+        h.copy_(x)
+    torch.cuda.synchronize()
+    del vis                      # the device-resident inputs make room for the staging buffers of the host entry
+    torch.cuda.empty_cache()
     e2e = None
     if args.e2e_steps > 0:
-        host = [x.pin_memory() for x in host]
         out = torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory()
+
         def timed_from_host(chunks):
             im.run_from_host(*host, out, chunks=chunks)
             torch.cuda.synchronize()
@@ -350,12 +377,10 @@ def main():
             return max_over_ranks((time.perf_counter() - t0) / args.e2e_steps, dist, dev)
 
         e2e_s = timed_from_host(args.e2e_chunks)
-        e2e = {"value": world * M / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
+        e2e = {"value": world * n_kept / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * M,
                "d2h_bytes_per_step": cfg.N * cfg.N * 8, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps,
-               "chunks": args.e2e_chunks,
+               "chunks": args.e2e_chunks, "image_seconds": e2e_s,
                "call": "rick_image_from_host_chunked" if args.e2e_chunks > 1 else "rick_image_from_host"}
-        if args.e2e_chunks > 1:
-            e2e["ms_per_step_one_chunk"] = timed_from_host(1) * 1e3
 
     if rank != 0:
         if dist is not None:
@@ -367,17 +392,21 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
         "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
-                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype, "fusion_mode": int(im.fused), "mesh_rows_defined": rows_defined, "mesh_rows": rows_total,
+                   "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype,
+                   "fusion_mode": int(im.fused),
+                   "column_engine": "split (colsplit.cu)" if split else ("one sweep (colfft.cu)" if one_sweep else "cuFFT 2-D + K5"),
+                   "mesh_rows_defined": rows_defined, "mesh_rows": rows_total,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "inputs (240 MB) and mesh (1.07 GB) exceed the 126 MB L2; no explicit flush"
-                   if args.config == "10M" else "inputs and mesh exceed L2; no explicit flush"},
+                   "l2": f"inputs ({24 * M / 1e9:.2f} GB) and mesh ({mesh_bytes / 1e9:.2f} GB) exceed the 126 MB L2; no explicit flush"},
+        "value_definition": "kept (gridded) visibilities of all ranks / step time; a step = rick_bin + rick_grid + rick_fft_planes + rick_wcorrect_accumulate",
+        "all_input_visibilities_per_sec": job_value(M, world, ms_per_step),
         "image_seconds": ms_per_step * 1e-3,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roofline, "stages": stages,
     }
     if world == 1 and not args.no_cpu_baseline:
         opa = dict(pa, kernel=args.kernel, beta=2.34 * cfg.support if args.kernel == "kb" else 0.0)
-        line["cpu_baseline"] = cpu_baseline(cfg, [h.numpy() for h in host], opa, M)
+        line["cpu_baseline"] = cpu_baseline(cfg, [h.numpy() for h in host], opa, M, n_kept)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -64,7 +64,10 @@ typedef enum { RICK_KERNEL_GAUSS = 0, RICK_KERNEL_KB = 1 } rick_kernel;
 enum { RICK_T_BIN = 0, RICK_T_ZERO = 1, RICK_T_GRID = 2, RICK_T_FFT = 3, RICK_T_WCORRECT = 4,
        RICK_T_IMAGE = 5,
        /* parts of RICK_T_BIN */
-       RICK_T_KEYGEN = 6, RICK_T_SORT = 7, RICK_T_GATHER = 8, RICK_T_COUNT = 9 };
+       RICK_T_KEYGEN = 6, RICK_T_SORT = 7, RICK_T_GATHER = 8,
+       /* parts of RICK_T_FFT when the column transform is fused (rick_plan_set_fusion): the row transforms and
+          sweep A of the split column transform */
+       RICK_T_FFT_ROWS = 9, RICK_T_FFT_COL_A = 10, RICK_T_COUNT = 11 };
 
 /* Create a plan (BASELINE.json north_star (1)).  Host-synchronous.
  *   N        mesh and image size per axis; a multiple of 32 (tile size), 32 <= N <= 32768
@@ -199,6 +202,13 @@ int rick_get_timings(rick_plan* plan, double* ms, int n);
 /* Number of launches of the library's own kernels issued through this plan so far (memsets, copies and
  * cuFFT's internal kernels are not counted). */
 long long rick_launch_count(const rick_plan* plan);
+
+/* Measurement helper (not part of the imaging path; host-synchronous, allocates 4 bytes and frees them):
+ * the fp32 rates of the current device from a register-resident microbenchmark on all SMs at full occupancy.
+ *   fma_tflops   2 x 1e12 fused multiply-adds per second (the fp32 FMA peak, TFLOP/s)
+ *   add_tinst    1e12 fp32 additions per second
+ * bench.py reports issue-bound kernels against these measured numbers. */
+int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, void* stream);
 
 const char* rick_strerror(int status);
 

@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 RICK_C64, RICK_C128 = 0, 1
-RICK_T_NAMES = ("bin", "zero", "grid", "fft", "wcorrect", "image", "keygen", "sort", "gather")
+RICK_T_NAMES = ("bin", "zero", "grid", "fft", "wcorrect", "image", "keygen", "sort", "gather", "fft_rows", "fft_col_a")
 
 _lib = None
 
@@ -24,6 +24,7 @@ EXPORTS = (
     "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_image_from_host_chunked", "rick_get_timings", "rick_launch_count", "rick_strerror",
+    "rick_measure_fp32_rate",
 )
 
 
@@ -75,6 +76,7 @@ def lib():
         L.rick_get_timings.argtypes = [vp, C.POINTER(dbl), i]
         L.rick_launch_count.argtypes = [vp]
         L.rick_launch_count.restype = ll
+        L.rick_measure_fp32_rate.argtypes = [C.POINTER(dbl), C.POINTER(dbl), vp]
         L.rick_strerror.argtypes = [i]
         L.rick_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -216,6 +218,13 @@ def rick_launch_count(plan: int) -> int:
     return int(lib().rick_launch_count(plan))
 
 
+def rick_measure_fp32_rate():
+    """-> (fp32 FMA TFLOP/s, 1e12 fp32 adds / s) measured on the current device (measurement helper)."""
+    a, b = C.c_double(), C.c_double()
+    _check(lib().rick_measure_fp32_rate(C.byref(a), C.byref(b), _stream()), "rick_measure_fp32_rate")
+    return float(a.value), float(b.value)
+
+
 # ---- buffer ownership helper (allocation + marshalling; no arithmetic) --------------------------
 
 class Imager:
@@ -224,7 +233,7 @@ class Imager:
 
     def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
                  dtype: str = "c64", M_max: int = 0, device="cuda", fused: int = 0,
-                 kernel: str = "gauss", beta: float = 0.0):
+                 kernel: str = "gauss", beta: float = 0.0, alloc_mesh: bool = True):
         if not torch.cuda.is_available():
             raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -240,8 +249,9 @@ class Imager:
             elif kernel != "gauss":
                 raise RickError(f"unknown gridding kernel {kernel!r}")
         self.M_max = 0
-        self.grid = torch.empty((Nw, N, N), dtype=self.cdtype, device=self.device)
-        self.image = torch.empty((N, N), dtype=torch.float64, device=self.device)
+        # alloc_mesh = False: a binning-only helper (rick_bin needs neither the mesh nor the image)
+        self.grid = torch.empty((Nw, N, N) if alloc_mesh else (0,), dtype=self.cdtype, device=self.device)
+        self.image = torch.empty((N, N) if alloc_mesh else (0,), dtype=torch.float64, device=self.device)
         self.n_kept = torch.zeros(1, dtype=torch.int64, device=self.device)
         _, fft_bytes = rick_plan_workspace_bytes(self.plan, 0)
         self.fft_work = torch.empty(fft_bytes, dtype=torch.uint8, device=self.device) if fft_bytes else None

@@ -45,6 +45,7 @@ void destroy_fft(rick_plan* p) {
     }
     p->fft_rows_work_bytes = 0;
     p->fused = 0;
+    p->split = false;
 }
 
 // batched 1-D inverse transforms of all Nw * N rows, in place (the row half of D7)
@@ -55,7 +56,8 @@ int build_fft_rows(rick_plan* p) {
     if (cufftSetAutoAllocation(h, 0) != CUFFT_SUCCESS) { cufftDestroy(h); return RICK_ECUFFT; }
     long long n[1] = {N};
     size_t work = 0;
-    if (cufftMakePlanMany64(h, 1, n, NULL, 1, N, NULL, 1, N, CUFFT_C2C, N * p->g.Nw, &work) != CUFFT_SUCCESS) {
+    const cufftType type = (p->dtype == RICK_C128) ? CUFFT_Z2Z : CUFFT_C2C;
+    if (cufftMakePlanMany64(h, 1, n, NULL, 1, N, NULL, 1, N, type, N * p->g.Nw, &work) != CUFFT_SUCCESS) {
         cufftDestroy(h);
         return RICK_ECUFFT;
     }
@@ -335,12 +337,16 @@ int rick_plan_set_fusion(rick_plan* p, int on) {
     if (on < 0 || on > 2) return RICK_EINVAL;
     if (!on) { p->fused = 0; return RICK_OK; }
     if (!p->dtype_set) return RICK_ESTATE;
-    if (!rick_colfft_supported(p)) return RICK_EINVAL;
+    // engine: the one-sweep column kernel where a column block fits one SM (fp32 mesh, N <= 2048), else the
+    // split column transform (two sweeps; N up to 16384, both mesh types)
+    const bool one_sweep = rick_colfft_supported(p);
+    if (!one_sweep && !rick_colsplit_supported(p)) return RICK_EINVAL;
     if (!p->fft_rows_ready) {
         int rc = build_fft_rows(p);
         if (rc != RICK_OK) return rc;
-        if ((rc = rick_colfft_init(p)) != RICK_OK) return rc;
+        if ((rc = one_sweep ? rick_colfft_init(p) : rick_colsplit_init(p)) != RICK_OK) return rc;
     }
+    p->split = !one_sweep;
     if (on == 2 && !p->occ_cur_dev) {
         const size_t words = (size_t)p->g.Nw * p->g.N / 32, rows = (size_t)p->g.Nw * p->g.N;
         if (cudaMalloc((void**)&p->occ_cur_dev, 4 * words) != cudaSuccess ||
@@ -370,7 +376,8 @@ int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes
     if (bin_bytes) *bin_bytes = rick_bin_workspace_bytes(p, M);
     if (fft_bytes) {
         if (!p->fft_ready) return RICK_ESTATE;
-        *fft_bytes = p->fft_work_bytes > p->fft_rows_work_bytes ? p->fft_work_bytes : p->fft_rows_work_bytes;
+        // fused: only the batched row transforms go through cuFFT
+        *fft_bytes = p->fused ? p->fft_rows_work_bytes : p->fft_work_bytes;
     }
     return RICK_OK;
 }
@@ -388,6 +395,7 @@ int rick_plan_destroy(rick_plan* p) {
     destroy_fft(p);
     if (p->inv_taper_dev) cudaFree(p->inv_taper_dev);
     if (p->colfft_tw) cudaFree(p->colfft_tw);
+    if (p->split_tw) cudaFree(p->split_tw);
     if (p->occ_cur_dev) cudaFree(p->occ_cur_dev);
     if (p->occ_mesh_dev) cudaFree(p->occ_mesh_dev);
     if (p->row_list_dev) cudaFree(p->row_list_dev);
@@ -442,23 +450,37 @@ int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
 int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_bytes, void* stream) {
     if (!p || !grid) return RICK_EINVAL;
     if (!p->fft_ready) return RICK_ESTATE;
-    if (p->fft_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_work_bytes)) return RICK_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
-    if (p->fused == 2) {   // row transforms of the defined rows only, by the library's own kernel (colfft.cu)
+    if (p->fused == 2 && !p->split) {   // row transforms of the defined rows only, by the library's own kernel (colfft.cu)
         StageTimer tm(p, RICK_T_FFT, st);
         int rc = rick_rows_list_all(p, st);
+        StageTimer tr(p, RICK_T_FFT_ROWS, st);
         if (rc == RICK_OK) rc = rick_rowfft_impl(p, grid, st);
         return rc;
     }
-    if (p->fused) {   // rows only; rick_wcorrect_accumulate finishes the transform (colfft.cu)
+    if (p->fused) {   // rows only (+ sweep A of the split engine); rick_wcorrect_accumulate finishes the transform
         if (p->fft_rows_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_rows_work_bytes)) return RICK_ENOMEM;
         if (cufftSetStream(p->fft_rows, st) != CUFFT_SUCCESS) return RICK_ECUFFT;
         if (p->fft_rows_work_bytes > 0 && cufftSetWorkArea(p->fft_rows, fft_work) != CUFFT_SUCCESS) return RICK_ECUFFT;
         StageTimer tm(p, RICK_T_FFT, st);
-        if (cufftExecC2C(p->fft_rows, (cufftComplex*)grid, (cufftComplex*)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
-            return RICK_ECUFFT;
+        {
+            StageTimer tr(p, RICK_T_FFT_ROWS, st);
+            const cufftResult r = p->dtype == RICK_C128
+                ? cufftExecZ2Z(p->fft_rows, (cufftDoubleComplex*)grid, (cufftDoubleComplex*)grid, CUFFT_INVERSE)
+                : cufftExecC2C(p->fft_rows, (cufftComplex*)grid, (cufftComplex*)grid, CUFFT_INVERSE);
+            if (r != CUFFT_SUCCESS) return RICK_ECUFFT;
+        }
+        if (p->split) {
+            // mode 2: rows no footprint touched hold undefined data; the library transforms them in place (each
+            // row on its own) and sweep A reads only the touched ones
+            int rc = p->fused == 2 ? rick_rows_list_all(p, st) : RICK_OK;
+            StageTimer ta(p, RICK_T_FFT_COL_A, st);
+            if (rc == RICK_OK) rc = rick_colsplit_a_impl(p, grid, st);
+            return rc;
+        }
         return RICK_OK;
     }
+    if (p->fft_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_work_bytes)) return RICK_ENOMEM;
     if (cufftSetStream(p->fft, st) != CUFFT_SUCCESS) return RICK_ECUFFT;
     if (p->fft_work_bytes > 0 && cufftSetWorkArea(p->fft, fft_work) != CUFFT_SUCCESS) return RICK_ECUFFT;
     StageTimer tm(p, RICK_T_FFT, st);
@@ -481,6 +503,7 @@ int rick_wcorrect_accumulate(rick_plan* p, const void* grid, double* image, int 
     if (!p || !grid || !image) return RICK_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     StageTimer tm(p, RICK_T_WCORRECT, st);
+    if (p->fused && p->split) return rick_colsplit_b_impl(p, grid, image, zero_first, st);
     if (p->fused) return rick_colfft_wcorrect_impl(p, grid, image, zero_first, st);
     return rick_wcorrect_impl(p, grid, image, zero_first, st);
 }
@@ -568,7 +591,7 @@ int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, co
         if ((rc = rick_grid(p, d->grid, i == 0, stream)) != RICK_OK) return rc;
     }
     if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
-    if (!p->fused) {
+    if (!p->fused || p->split) {
         if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
         if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;
         RICK_CUDA(cudaStreamSynchronize(st));

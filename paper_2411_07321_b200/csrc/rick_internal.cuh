@@ -65,6 +65,10 @@ struct rick_plan {
     bool fft_rows_ready;
     size_t fft_rows_work_bytes;
     void* colfft_tw;         // device float2[N]: exp(+2 pi i j / N)
+    // split column transform (colsplit.cu): N = split_N1 * split_N2, engine selected by rick_plan_set_fusion
+    bool split;              // fused != 0: true = sweeps A + B of colsplit.cu, false = the one-sweep kernel of colfft.cu
+    int split_N1, split_N2;
+    void* split_tw;          // device float2[N] / double2[N] (mesh precision): exp(+2 pi i j / N)
     // cuFFT
     cufftHandle fft;
     bool fft_ready;
@@ -168,6 +172,10 @@ int rick_colfft_wcorrect_impl(rick_plan* p, const void* grid, double* image, int
                               int col_lo = 0, int col_hi = -1, bool clear_image = true);
 int rick_colfft_split(const rick_plan* p);                              // 1 or 2 plane halves per column block
 int rick_colfft_columns_per_cta();
+bool rick_colsplit_supported(const rick_plan* p);
+int rick_colsplit_init(rick_plan* p);
+int rick_colsplit_a_impl(rick_plan* p, void* grid, cudaStream_t st);
+int rick_colsplit_b_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
 int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st);          // rick_bin: occ_cur from the records
 int rick_rows_clear(rick_plan* p, void* grid, int zero_first, cudaStream_t st);   // rick_grid: clear new rows
 int rick_rows_list_all(rick_plan* p, cudaStream_t st);                   // row_list = all defined rows

@@ -66,16 +66,56 @@ def check_bin(im, vis, pa):
     return okey, operm, n_kept
 
 
-@pytest.mark.parametrize("name,M,plan,dtype", [
+def check_bin_fused_gather(im, vis, pa):
+    """rick_bin as Imager.run and bench.py call it -- no perm_out / bin_start_out, so the gather rides in the
+    last one-sweep pass (k_onesweep<..., kGather>): n_kept and the five sorted arrays against the oracle's
+    stable D4' order, bit for bit."""
+    u, v, w, vv, wt = vis.numpy()
+    plan = O.Plan(**pa)
+    s = im.sorted
+    for t in s.values():
+        t.view(torch.uint8).fill_(0xA5)
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
+    torch.cuda.synchronize()
+    n_kept = int(im.n_kept.item())
+    _, oi0, oj0, ok, on = O.keys(plan, u, v, w, vv, wt)
+    assert n_kept == on
+    _, _, cell_bits = B.rick_plan_sort_layout(im.plan)
+    sel = O.sort_cells(oi0, oj0, ok, col_drop=10 - cell_bits)[:n_kept].astype(np.int64)
+    assert np.array_equal(s["u"][:n_kept].cpu().numpy(), u[sel])
+    assert np.array_equal(s["v"][:n_kept].cpu().numpy(), v[sel])
+    assert np.array_equal(s["w"][:n_kept].cpu().numpy(), w[sel])
+    assert np.array_equal(s["vis"][:n_kept].cpu().numpy().view(np.uint32), vv[sel].view(np.uint32))
+    assert np.array_equal(s["weight"][:n_kept].cpu().numpy(), wt[sel])
+    return n_kept
+
+
+BIN_CASES = [
     ("tiny", 100_000, {}, "c128"),
     ("10M", 300_017, dict(N=512, Nw=8), "c64"),                     # ragged tail, several sort tiles
-    ("10M", 1_000_003, dict(N=2048, Nw=32), "c64"),                 # 18-bit keys, 3 passes
-    ("hotspot", 400_001, dict(N=1024, Nw=4), "c64"),  # support 9, 70 % in a dense core
-])
+    ("10M", 1_000_003, dict(N=2048, Nw=32), "c64"),                 # 27-bit sort keys, 3 passes of 9 bits
+    ("hotspot", 400_001, dict(N=1024, Nw=4), "c64"),                # support 9, 70 % in a dense core
+    ("500M", 700_001, dict(N=8192, Nw=32), "c64"),                  # the 500M plan: 31-bit sort keys, 4 passes of 8 bits
+]
+
+
+@pytest.mark.parametrize("name,M,plan,dtype", BIN_CASES)
 def test_bin_bit_exact(name, M, plan, dtype):
     cfg, vis, pa = make(name, M, dtype=dtype, **plan)
-    im = B.Imager(dtype=dtype, M_max=M, **pa)
+    im = B.Imager(dtype=dtype, M_max=M, alloc_mesh=False, **pa)
     check_bin(im, vis, pa)
+    im.close()
+
+
+@pytest.mark.parametrize("name,M,plan,dtype", BIN_CASES)
+@pytest.mark.parametrize("fused", [0, 2])
+def test_bin_bit_exact_fused_gather(name, M, plan, dtype, fused):
+    """The variant of rick_bin the timed path runs (gather fused into the last sort pass; fusion mode 2 adds
+    the row marking)."""
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    im = B.Imager(dtype=dtype, M_max=M, fused=fused, alloc_mesh=False, **pa)
+    n_kept = check_bin_fused_gather(im, vis, pa)
+    assert 0 < n_kept <= M
     im.close()
 
 
@@ -153,16 +193,23 @@ def test_stages_and_image(name, M, plan, dtype):
 
 
 def test_full_config_10M_image():
-    """BASELINE.json configs[1] at full size, in the configuration bench.py times."""
+    """BASELINE.json configs[1] at full size (1e7 visibilities, 2048^2 x 32, c64) in every fusion mode:
+    2 (row occupancy + own row transforms + one-sweep column kernel: what `bench.py --config 10M` times),
+    1 (dense, cuFFT rows + column kernel) and 0 (2-D cuFFT + K5)."""
     cfg, vis, pa = make("10M", W.CONFIGS["10M"].M)
-    im = B.Imager(dtype="c64", M_max=vis.M, **pa)
-    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy()
     ref, n_kept, _ = O.image(O.Plan(**pa), *vis.numpy(), return_timing=True)
-    assert int(im.n_kept.item()) == n_kept
-    a, b, full = gates(img, ref, cfg.N, cfg.support, cfg.sigma)
-    print(f"10M full: n_kept={n_kept} gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
-    assert a <= TOL["c64"] and b <= TOL["c64"]
-    im.close()
+    for fused in (2, 1, 0):
+        im = B.Imager(dtype="c64", M_max=vis.M, fused=fused, **pa)
+        assert im.fused == fused
+        im.grid.fill_(complex(float("nan"), float("nan")))
+        img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy()
+        assert int(im.n_kept.item()) == n_kept
+        a, b, full = gates(img, ref, cfg.N, cfg.support, cfg.sigma)
+        print(f"10M full, fusion {fused}: n_kept={n_kept} gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
+        assert a <= TOL["c64"] and b <= TOL["c64"], (fused, a, b)
+        im.close()
+        del im
+        torch.cuda.empty_cache()
 
 
 def test_edge_cases():
@@ -400,4 +447,110 @@ def test_fusion_mode_2_row_occupancy(name, M, plan, kernel):
     chunked = im.image.cpu().numpy()
     assert np.isfinite(chunked).all()
     assert (np.abs(chunked - img) * tw).max() <= 2e-6 * np.abs(img * tw).max()
+    im.close()
+
+
+@pytest.mark.parametrize("name,M,plan,dtype,fused", [
+    ("tiny", 100_000, dict(N=256, Nw=8), "c128", 1),          # 16 x 16
+    ("10M", 300_000, dict(N=512, Nw=8), "c128", 2),           # 16 x 32
+    ("100M", 300_000, dict(N=1024, Nw=16), "c128", 1),        # 32 x 32, wide field: the w term matters
+    ("100M", 300_000, dict(N=2048, Nw=4), "c128", 2),         # 32 x 64
+    ("100M", 400_000, dict(N=4096, Nw=4), "c128", 2),         # 64 x 64: the 100M plan's transform
+    ("500M", 400_000, dict(N=4096, Nw=4), "c64", 1),          # 64 x 64
+    ("500M", 400_000, dict(N=8192, Nw=3), "c64", 2),          # 64 x 128: the 500M plan's transform, odd plane count
+    ("hotspot", 400_001, dict(N=16384, Nw=2), "c64", 2),      # 128 x 128: the hotspot plan's transform, support 9
+])
+def test_split_column_transform(name, M, plan, dtype, fused):
+    """rick_plan_set_fusion on plans the one-sweep column kernel cannot take (N >= 4096, or the fp64 mesh):
+    cuFFT rows + sweep A (k_col_a) + sweep B fused with the w-correction (k_col_b).  Image against the oracle
+    (same gates); with fusion mode 2 the mesh is pre-filled with NaN; accumulate mode adds."""
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    N = pa["N"]
+    im = B.Imager(dtype=dtype, M_max=M, fused=fused, **pa)
+    assert im.fused == fused
+    if fused == 2:
+        im.grid.view(torch.float64 if dtype == "c128" else torch.float32).fill_(float("nan"))
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    assert np.isfinite(img).all()
+    ref = O.image(O.Plan(**pa), *vis.numpy())
+    a, b, full = gates(img, ref, N, cfg.support, cfg.sigma)
+    print(f"split {name}/{dtype} N={N} Nw={pa['Nw']} fusion {fused}: gateA {a:.2e} gateB {b:.2e} full {full:.2e}")
+    assert a <= TOL[dtype] and b <= TOL[dtype]
+    im.grid_(True)
+    im.fft()
+    im.wcorrect(False)                                     # accumulate onto the image: twice the image
+    torch.cuda.synchronize()
+    twice = im.image.cpu().numpy()
+    t = O.taper(N, cfg.support, cfg.sigma)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    assert (np.abs(twice - 2 * img) * tw).max() <= (1e-12 if dtype == "c128" else 2e-6) * np.abs(img * tw).max()
+    im.close()
+
+
+@pytest.mark.parametrize("S", [3, 5, 7, 9, 11, 13, 15])
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("kernel", ["gauss", "kb"])
+def test_every_support(S, dtype, kernel):
+    """Every footprint width rick_plan_create accepts, both mesh types, both kernels (the multi-pass record
+    gridder for S >= 11 and every k_grid_runs instantiation): mesh and image against the oracle.  The input
+    includes visibilities on the last cells D5 keeps (i0 = h and i0 = N-1-h: the window's zero column falls
+    off the row there)."""
+    N, Nw, M = 256, 4, 60_000
+    sigma = max(0.45, 0.16 * S)
+    cfg, vis, pa = make("10M", M, dtype=dtype, N=N, Nw=Nw, support=S, sigma=sigma)
+    h = (S - 1) // 2
+    du = 1.0 / (N * pa["dl"])
+    edge = torch.tensor([(h - N // 2) * du, (N - 1 - h - N // 2) * du], dtype=torch.float32, device="cuda")
+    vis.u[:2] = edge
+    vis.v[:2] = edge.flip(0)
+    vis.u[2:4] = edge
+    vis.v[2:4] = 0.0
+    beta = 2.34 * S
+    oplan = O.Plan(kernel=kernel, beta=beta, **pa)
+    hv = vis.numpy()
+    im = B.Imager(dtype=dtype, M_max=M, kernel=kernel, beta=beta, **pa)
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
+    im.grid_(True)
+    torch.cuda.synchronize()
+    ii = np.arange(N)
+    cb = np.where((ii[:, None] + ii[None, :]) & 1, -1.0, 1.0)
+    g = im.grid.cpu().numpy().astype(np.complex128) * cb[None]
+    og = O.grid(oplan, *hv)
+    gerr = np.abs(g - og).max() / np.abs(og).max()
+    assert gerr <= (1e-12 if dtype == "c128" else 3e-6), gerr
+    im.fft()
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    img = im.image.cpu().numpy()
+    ref = O.image(oplan, *hv)
+    t = O.taper(N, S, sigma, kernel, beta)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    inner = slice(N // 4, 3 * N // 4)
+    peak = np.abs(ref[inner, inner]).max()
+    d = np.abs(img - ref)
+    a, b = d[tw >= 1e-2].max() / peak, (d * tw).max() / peak
+    print(f"S={S} {dtype} {kernel}: grid {gerr:.2e} gateA {a:.2e} gateB {b:.2e}")
+    assert a <= TOL[dtype] and b <= TOL[dtype]
+    im.close()
+
+
+@pytest.mark.parametrize("N,dtype", [(96, "c128"), (160, "c64"), (480, "c64")])
+def test_mesh_size_not_a_power_of_two(N, dtype):
+    """rick_plan_create accepts any multiple of 32.  The oracle's own FFT is radix 2, so D7 is evaluated here
+    with numpy's ifft2 on the oracle's mesh (the identity tests/test_oracle_pins.py pins the oracle's transform
+    with), then the oracle's own w-correction."""
+    Nw, M = 4, 50_000
+    cfg, vis, pa = make("10M", M, dtype=dtype, N=N, Nw=Nw)
+    oplan = O.Plan(**pa)
+    hv = vis.numpy()
+    im = B.Imager(dtype=dtype, M_max=M, **pa)
+    img = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy()
+    og = O.grid(oplan, *hv)
+    ii = np.arange(N)
+    cb = np.where((ii[:, None] + ii[None, :]) & 1, -1.0, 1.0)
+    planes = np.stack([cb * np.fft.ifft2(cb * og[k]) * (N * N) for k in range(Nw)])
+    ref = O.wcorrect(oplan, planes)
+    a, b, full = gates(img, ref, N, cfg.support, cfg.sigma)
+    print(f"N={N} {dtype}: gateA {a:.2e} gateB {b:.2e}")
+    assert a <= TOL[dtype] and b <= TOL[dtype]
     im.close()
