@@ -206,6 +206,8 @@ def main():
                     help="rick_plan_set_fusion mode: 1 fused column transform, 2 + row occupancy")
     ap.add_argument("--kernel", default="gauss", choices=["gauss", "kb"],
                     help="gridding kernel: the Gaussian of BASELINE.json (default) or the paper's Kaiser-Bessel (beta = 2.34 S)")
+    ap.add_argument("--M", type=int, default=0, help="profiling subset: only the first M visibilities of the workload")
+    ap.add_argument("--Nw", type=int, default=0, help="profiling subset: this many w-planes instead of the workload's")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-chunks", type=int, default=4,
                     help="time slices of rick_image_from_host_chunked in the e2e region (1: one copy, then compute)")
@@ -233,13 +235,15 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = W.CONFIGS[args.config]
+    if args.M or args.Nw:       # a subset for profiler captures (ncu saves and restores what a kernel writes); not a bench line
+        cfg = W.scaled(cfg, args.M or cfg.M, Nw=args.Nw or cfg.Nw)
     vis = W.generate(cfg, device=dev)
     pa = W.plan_args(cfg, vis)
     M = vis.M
     im = B.Imager(dtype=cfg.dtype, M_max=M, fused=0 if args.no_fusion else args.fusion, kernel=args.kernel, beta=2.34 * cfg.support, **pa)
     cell = 16 if cfg.dtype == "c128" else 8
     mesh_bytes = cfg.Nw * cfg.N * cfg.N * cell
-    fma_tflops, add_tinst = B.rick_measure_fp32_rate()
+    fma_tflops, add_tinst, fma2_tflops = B.rick_measure_fp32_rate()
 
     def step():
         im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight)
@@ -294,7 +298,8 @@ def main():
         fft_rows_b = 2 * live_bytes          # mode 2: own row kernel on the defined rows; mode 1: live = mesh
         col_a_b, fft_b, wc_b = 0, fft_rows_b, live_bytes + cfg.N * cfg.N * 8
     else:
-        fft_rows_b = 2 * mesh_bytes          # batched library row transforms of every row
+        own_rows = im.fused == 2 and cfg.N >= 4096 and not (cfg.dtype == "c128" and cfg.N > 8192)   # rowbig.cu
+        fft_rows_b = 2 * live_bytes if own_rows else 2 * mesh_bytes      # else batched library transforms of every row
         col_a_b = live_bytes + mesh_bytes    # sweep A reads the defined rows, writes every row
         fft_b, wc_b = fft_rows_b + col_a_b, mesh_bytes + cfg.N * cfg.N * 8
     alg = {   # algorithmic bytes per stage
@@ -328,6 +333,8 @@ def main():
                "wcorrect": ("k_col_b" if split else ("k_colfft_wcorrect" if one_sweep else "k_wcorrect"), 1)}
     if split:
         kernels["fft_col_a"] = ("k_col_a", 1)
+        if own_rows:
+            kernels["fft_rows"] = ("k_row_big", 1)
     elif one_sweep and im.fused == 2:
         kernels["fft_rows"] = ("k_rowfft", 1)
     dom = max(kernels, key=lambda k: stage_ms[k])
@@ -343,7 +350,8 @@ def main():
     # instruction-issue view of the transform kernels against the fp32 rates measured in this run
     # (rick_measure_fp32_rate: a register-resident FMA / ADD chain on every SM), 5 L log2 L flop per L-point transform
     import math
-    alu = {"fp32_fma_tflops_measured": fma_tflops, "fp32_add_tinst_measured": add_tinst}
+    alu = {"fp32_fma_tflops_measured": fma_tflops, "fp32_add_tinst_measured": add_tinst,
+           "fp32x2_fma_tflops_measured": fma2_tflops}
     if cfg.dtype == "c64" and im.fused:
         n_el = cfg.N * cfg.N * cfg.Nw
         if one_sweep:
@@ -391,7 +399,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
-        "config": {"workload": args.config, "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
+        "config": {"workload": args.config + (" (profiling subset)" if args.M or args.Nw else ""), "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
                    "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype,
                    "fusion_mode": int(im.fused),
                    "column_engine": "split (colsplit.cu)" if split else ("one sweep (colfft.cu)" if one_sweep else "cuFFT 2-D + K5"),

@@ -207,8 +207,9 @@ long long rick_launch_count(const rick_plan* plan);
  * the fp32 rates of the current device from a register-resident microbenchmark on all SMs at full occupancy.
  *   fma_tflops   2 x 1e12 fused multiply-adds per second (the fp32 FMA peak, TFLOP/s)
  *   add_tinst    1e12 fp32 additions per second
+ *   fma2_tflops  the same FMA chain with the packed fma.rn.f32x2 of sm_100 (4 flop per lane-op), TFLOP/s
  * bench.py reports issue-bound kernels against these measured numbers. */
-int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, void* stream);
+int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, double* fma2_tflops, void* stream);
 
 const char* rick_strerror(int status);
 

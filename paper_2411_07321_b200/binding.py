@@ -76,7 +76,7 @@ def lib():
         L.rick_get_timings.argtypes = [vp, C.POINTER(dbl), i]
         L.rick_launch_count.argtypes = [vp]
         L.rick_launch_count.restype = ll
-        L.rick_measure_fp32_rate.argtypes = [C.POINTER(dbl), C.POINTER(dbl), vp]
+        L.rick_measure_fp32_rate.argtypes = [C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), vp]
         L.rick_strerror.argtypes = [i]
         L.rick_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -219,10 +219,10 @@ def rick_launch_count(plan: int) -> int:
 
 
 def rick_measure_fp32_rate():
-    """-> (fp32 FMA TFLOP/s, 1e12 fp32 adds / s) measured on the current device (measurement helper)."""
-    a, b = C.c_double(), C.c_double()
-    _check(lib().rick_measure_fp32_rate(C.byref(a), C.byref(b), _stream()), "rick_measure_fp32_rate")
-    return float(a.value), float(b.value)
+    """-> (fp32 FMA TFLOP/s, 1e12 fp32 adds / s, packed-FMA TFLOP/s) measured on the current device."""
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().rick_measure_fp32_rate(C.byref(a), C.byref(b), C.byref(c), _stream()), "rick_measure_fp32_rate")
+    return float(a.value), float(b.value), float(c.value)
 
 
 # ---- buffer ownership helper (allocation + marshalling; no arithmetic) --------------------------

@@ -42,15 +42,22 @@ template <int L> __host__ __device__ constexpr int slot_freq(int slot) {
     return Split<L>::R2 == 1 ? slot : (slot / Split<L>::R2) + Split<L>::R1 * (slot % Split<L>::R2);
 }
 
-template <typename C2> RICK_DI C2 ldg_cx(const C2* p);
-template <> RICK_DI float2 ldg_cx<float2>(const float2* p) {
+// streaming load of one complex value when `live`, else zero -- predicated, no branch
+template <typename C2> RICK_DI C2 ldg_cx_if(const C2* p, bool live);
+template <> RICK_DI float2 ldg_cx_if<float2>(const float2* p, bool live) {
     float2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+                 "mov.f32 %0, 0f00000000;\n\tmov.f32 %1, 0f00000000;\n\t"
+                 "@q ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];\n\t}"
+                 : "=&f"(r.x), "=&f"(r.y) : "l"(p), "r"((unsigned)live));
     return r;
 }
-template <> RICK_DI double2 ldg_cx<double2>(const double2* p) {
+template <> RICK_DI double2 ldg_cx_if<double2>(const double2* p, bool live) {
     double2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+                 "mov.f64 %0, 0d0000000000000000;\n\tmov.f64 %1, 0d0000000000000000;\n\t"
+                 "@q ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];\n\t}"
+                 : "=&d"(r.x), "=&d"(r.y) : "l"(p), "r"((unsigned)live));
     return r;
 }
 
@@ -66,41 +73,44 @@ template <int L, typename C2> RICK_DI void first_pass(C2* v, const C2* twL, int 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Sweep A
+// Sweep A.  N = N1 N2 is a compile-time constant: every row stride below is an immediate.
 // ---------------------------------------------------------------------------------------------
-template <typename C2, int L>
-__global__ void __launch_bounds__(L * ColsOf<C2>::C / Split<L>::R1)
-k_col_a(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* __restrict__ occ, int N, int N2) {
+template <typename C2, int N1, int N2>
+__global__ void __launch_bounds__(N1 * ColsOf<C2>::C / Split<N1>::R1)
+k_col_a(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* __restrict__ occ) {
+    constexpr int L = N1, N = N1 * N2;
     constexpr int R1 = Split<L>::R1, R2 = Split<L>::R2, C = ColsOf<C2>::C;
     constexpr int T = L * C / R1;
+    constexpr size_t rstride = (size_t)N2 * N;                          // mesh rows j2 + N2 j1 are N2 rows apart
     __shared__ C2 tile[R2 > 1 ? L * C : 1];
     __shared__ C2 twL[L];
+    __shared__ C2 twq[L];                                               // W_N^(j2 q1), q1 < N1
     const int tid = threadIdx.x, c = tid % C, g = tid / C;
     const int j2 = blockIdx.y, k = blockIdx.z;
-    const size_t rstride = (size_t)N2 * N;                              // mesh rows j2 + N2 j1 are N2 rows apart
     C2* base = planes + ((size_t)k * N + j2) * N + (size_t)blockIdx.x * C + c;
     C2 v[R1];
+    {
+        bool live[R1];
 #pragma unroll
-    for (int t = 0; t < R1; ++t) {
-        const int j1 = g + t * R2;
-        bool live = true;
-        if (occ) {
-            const uint32_t r = (uint32_t)k * (uint32_t)N + (uint32_t)(N2 * j1 + j2);
-            live = (__ldg(occ + (r >> 5)) >> (r & 31)) & 1u;
+        for (int t = 0; t < R1; ++t) {
+            live[t] = true;
+            if (occ) {
+                const uint32_t r = (uint32_t)k * (uint32_t)N + (uint32_t)(N2 * (g + t * R2) + j2);
+                live[t] = (__ldg(occ + (r >> 5)) >> (r & 31)) & 1u;
+            }
         }
-        v[t] = live ? ldg_cx(base + (size_t)j1 * rstride) : cx_make<C2>(0, 0);
+#pragma unroll
+        for (int t = 0; t < R1; ++t) v[t] = ldg_cx_if(base + (size_t)(g + t * R2) * rstride, live[t]);
     }
-    if (R2 > 1) {
-        for (int i = tid; i < L; i += T) twL[i] = tw_g[(size_t)i * (N / L)];
-        __syncthreads();
+    for (int i = tid; i < L; i += T) {
+        twL[i] = tw_g[i * N2];                                          // W_L^i = W_N^(i N / L)
+        twq[i] = tw_g[(j2 * i) & (N - 1)];
     }
+    __syncthreads();
     first_pass<L>(v, twL, g);
     if constexpr (R2 == 1) {
 #pragma unroll
-        for (int u = 0; u < R1; ++u) {                                  // slot u = frequency u
-            const C2 w = __ldg(tw_g + ((j2 * u) & (N - 1)));
-            base[(size_t)u * rstride] = cx_mul(v[u], w);
-        }
+        for (int u = 0; u < R1; ++u) base[(size_t)u * rstride] = cx_mul(v[u], twq[u]);      // slot u = frequency u
     } else {
 #pragma unroll
         for (int u = 0; u < R1; ++u) tile[(g + u * R2) * C + c] = v[u];
@@ -114,10 +124,8 @@ k_col_a(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* __
             for (int s = 0; s < R2; ++s) w[s] = tile[(u * R2 + s) * C + c];
             cx_dft<R2>(w);
 #pragma unroll
-            for (int s = 0; s < R2; ++s) {                              // slot u R2 + s holds q1 = u + R1 s
-                const C2 tw = __ldg(tw_g + ((j2 * (u + R1 * s)) & (N - 1)));
-                base[(size_t)(u * R2 + s) * rstride] = cx_mul(w[s], tw);
-            }
+            for (int s = 0; s < R2; ++s)                                // slot u R2 + s holds q1 = u + R1 s
+                base[(size_t)(u * R2 + s) * rstride] = cx_mul(w[s], twq[u + R1 * s]);
         }
     }
 }
@@ -183,32 +191,52 @@ template <int E> struct Screen<double, E> {
     }
 };
 
+// n - 1 = -(l^2 + m^2) / (1 + sqrt(1 - l^2 - m^2)) without the library's IEEE square root and division (two
+// subroutine calls per output): fp32 seeds refined by two Newton steps each in fp64 (error < 2 ulp; a thread
+// needs E of these before its first plane, which weighed 14 % of the kernel at 16 planes)
+RICK_DI double nm1_fast(double r2) {
+    const double y = 1.0 - r2;
+    double x = (double)rsqrtf((float)y);
+    x = x * fma(-0.5 * y, x * x, 1.5);
+    x = x * fma(-0.5 * y, x * x, 1.5);
+    const double d = fma(y, x, 1.0);                     // 1 + sqrt(y)
+    double r = (double)__frcp_rn((float)d);
+    r = r * fma(-d, r, 2.0);
+    r = r * fma(-d, r, 2.0);
+    return -r2 * r;
+}
+template <typename real> RICK_DI double nm1_of(double r2);
+template <> RICK_DI double nm1_of<float>(double r2) { return nm1_fast(r2); }
+template <> RICK_DI double nm1_of<double>(double r2) { return -r2 / (1.0 + sqrt(1.0 - r2)); }
+
 template <typename C2, int L> struct ColB {
     static constexpr int R1 = Split<L>::R1, R2 = Split<L>::R2, C = ColsOf<C2>::C;
     static constexpr int T = L * C / R1;
     static constexpr int kIssuers = L < T ? L : T;                // threads that issue row copies
     static constexpr int kRowsPerIssuer = L / kIssuers;
     static constexpr size_t smem = 2 * sizeof(C2) * L * C + sizeof(C2) * L + 2 * sizeof(unsigned long long);
+    // resident CTAs the register allocation must leave room for (two of 256 threads: <= 128 registers)
+    static constexpr int kMinBlocks = (sizeof(C2) == 16 && L == 128) ? 1 : (T >= 256 ? 2 : 3);
 };
 
-template <typename C2, int L>
-__global__ void __launch_bounds__(ColB<C2, L>::T)
+template <typename C2, int N1, int N2>
+__global__ void __launch_bounds__(ColB<C2, N2>::T, ColB<C2, N2>::kMinBlocks)
 k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, const double* __restrict__ inv_t,
-        double* __restrict__ image, int accumulate, int N1, int a_R1, int a_R2) {
+        double* __restrict__ image, int accumulate) {
     typedef typename RickRealOf<C2>::type real;
+    constexpr int L = N2, N = N1 * N2;
     typedef ColB<C2, L> P;
     constexpr int R1 = P::R1, R2 = P::R2, C = P::C, T = P::T, E = R1;
+    constexpr size_t plane_cells = (size_t)N * N;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C2* buf0 = reinterpret_cast<C2*>(smem_raw);
     C2* buf1 = buf0 + L * C;
     C2* twL = buf1 + L * C;
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(twL + L);
     const int tid = threadIdx.x, c = tid % C, gq = tid / C;
-    const int N = g.N;
     const int b = blockIdx.y;                                       // block of L consecutive mesh rows
-    const int q1 = a_R2 == 1 ? b : (b / a_R2) + a_R1 * (b % a_R2);  // the frequency sweep A left there
+    const int q1 = slot_freq<N1>(b);                                // the frequency sweep A left there
     const int col0 = blockIdx.x * C, p = col0 + c;
-    const size_t plane_cells = (size_t)N * N;
     const C2* src0 = planes + (size_t)b * L * N + col0;             // row 0 of the tile in plane 0
 
     if (tid == 0) {
@@ -216,7 +244,7 @@ k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, 
         mbar_init(bar + 1, P::kIssuers);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = tid; i < L; i += T) twL[i] = tw_g[(size_t)i * (N / L)];
+    for (int i = tid; i < L; i += T) twL[i] = tw_g[i * N1];         // W_L^i = W_N^(i N / L)
     __syncthreads();
 
     auto issue = [&](int k) {
@@ -230,6 +258,8 @@ k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, 
             }
         }
     };
+    issue(0);
+    if (g.Nw > 1) issue(1);
 
     Screen<real, E> scr;
     double acc[E];
@@ -238,17 +268,16 @@ k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, 
         const int q2 = R2 == 1 ? e : (gq + R2 * (e / R2)) + R1 * (e % R2);
         return q1 + N1 * q2;
     };
+    {
+        const double l = (double)(p - N / 2) * g.dl, l2 = l * l;
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int q = out_q(e);
-        const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
-        const double r2 = l * l + m * m;
-        scr.init(e, -r2 / (1.0 + sqrt(1.0 - r2)), g);
-        acc[e] = 0.0;
+        for (int e = 0; e < E; ++e) {
+            const double m = (double)(out_q(e) - N / 2) * g.dl;
+            scr.init(e, nm1_of<real>(fma(m, m, l2)), g);
+            acc[e] = 0.0;
+        }
     }
 
-    issue(0);
-    if (g.Nw > 1) issue(1);
     for (int k = 0; k < g.Nw; ++k) {
         C2* buf = (k & 1) ? buf1 : buf0;
         const unsigned parity = (unsigned)(k >> 1) & 1u;
@@ -299,60 +328,56 @@ k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, 
     }
 }
 
-template <typename C2, int L>
+template <typename C2, int N1, int N2>
 int launch_a(rick_plan* p, void* grid, cudaStream_t st) {
-    constexpr int C = ColsOf<C2>::C, T = L * C / Split<L>::R1;
-    const int N = p->g.N, N2 = N / L;
+    constexpr int C = ColsOf<C2>::C, T = N1 * C / Split<N1>::R1, N = N1 * N2;
     const dim3 blocks((unsigned)(N / C), (unsigned)N2, (unsigned)p->g.Nw);
     const uint32_t* occ = p->fused == 2 ? p->occ_mesh_dev : nullptr;
-    k_col_a<C2, L><<<blocks, T, 0, st>>>((C2*)grid, (const C2*)p->split_tw, occ, N, N2);
+    k_col_a<C2, N1, N2><<<blocks, T, 0, st>>>((C2*)grid, (const C2*)p->split_tw, occ);
     return RICK_OK;
 }
 
-template <typename C2, int L>
+template <typename C2, int N1, int N2>
 int launch_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st) {
-    typedef ColB<C2, L> P;
+    typedef ColB<C2, N2> P;
+    constexpr int N = N1 * N2;
     static bool attr_done[RICK_MAX_DEVICES] = {};
     bool& done = attr_done[p->device & (RICK_MAX_DEVICES - 1)];
     if (!done) {
-        if (cudaFuncSetAttribute(k_col_b<C2, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_col_b<C2, N1, N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem) != cudaSuccess)
             return RICK_ECUDA;
         done = true;
     }
-    const int N = p->g.N, N1 = N / L;
     const dim3 blocks((unsigned)(N / P::C), (unsigned)N1);
-    int a_R1 = 0, a_R2 = 0;
-    switch (N1) {
-        case 16: a_R1 = Split<16>::R1; a_R2 = Split<16>::R2; break;
-        case 32: a_R1 = Split<32>::R1; a_R2 = Split<32>::R2; break;
-        case 64: a_R1 = Split<64>::R1; a_R2 = Split<64>::R2; break;
-        case 128: a_R1 = Split<128>::R1; a_R2 = Split<128>::R2; break;
-        default: return RICK_EINVAL;
-    }
-    k_col_b<C2, L><<<blocks, P::T, P::smem, st>>>(p->g, (const C2*)grid, (const C2*)p->split_tw, p->inv_taper_dev, image,
-                                                    accumulate, N1, a_R1, a_R2);
+    k_col_b<C2, N1, N2><<<blocks, P::T, P::smem, st>>>(p->g, (const C2*)grid, (const C2*)p->split_tw, p->inv_taper_dev,
+                                                        image, accumulate);
     return RICK_OK;
 }
 
+// the (N1, N2) pairs of N = 256 .. 16384
+#define RICK_SPLIT_DISPATCH(CALL)                                            \
+    switch (p->g.N) {                                                        \
+        case 256: return CALL(16, 16);                                       \
+        case 512: return CALL(16, 32);                                       \
+        case 1024: return CALL(32, 32);                                      \
+        case 2048: return CALL(32, 64);                                      \
+        case 4096: return CALL(64, 64);                                      \
+        case 8192: return CALL(64, 128);                                     \
+        case 16384: return CALL(128, 128);                                   \
+        default: return RICK_EINVAL;                                         \
+    }
+
 template <typename C2>
 int sweep_a(rick_plan* p, void* grid, cudaStream_t st) {
-    switch (p->split_N1) {
-        case 16: return launch_a<C2, 16>(p, grid, st);
-        case 32: return launch_a<C2, 32>(p, grid, st);
-        case 64: return launch_a<C2, 64>(p, grid, st);
-        case 128: return launch_a<C2, 128>(p, grid, st);
-        default: return RICK_EINVAL;
-    }
+#define RICK_CALL_A(n1, n2) launch_a<C2, n1, n2>(p, grid, st)
+    RICK_SPLIT_DISPATCH(RICK_CALL_A)
+#undef RICK_CALL_A
 }
 template <typename C2>
 int sweep_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st) {
-    switch (p->split_N2) {
-        case 16: return launch_b<C2, 16>(p, grid, image, accumulate, st);
-        case 32: return launch_b<C2, 32>(p, grid, image, accumulate, st);
-        case 64: return launch_b<C2, 64>(p, grid, image, accumulate, st);
-        case 128: return launch_b<C2, 128>(p, grid, image, accumulate, st);
-        default: return RICK_EINVAL;
-    }
+#define RICK_CALL_B(n1, n2) launch_b<C2, n1, n2>(p, grid, image, accumulate, st)
+    RICK_SPLIT_DISPATCH(RICK_CALL_B)
+#undef RICK_CALL_B
 }
 
 }  // namespace

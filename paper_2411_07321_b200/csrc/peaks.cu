@@ -23,10 +23,31 @@ __global__ void __launch_bounds__(256) k_fp32_rate(float* out, int n_iter, float
     if (s == 12345.678f) out[0] = s;      // keeps the chains alive; practically never true
 }
 
+// the same chain with the packed instruction of sm_100 (fma.rn.f32x2 -> FFMA2: two fused multiply-adds per lane)
+__global__ void __launch_bounds__(256) k_fp32x2_rate(float* out, int n_iter, float a, float b) {
+    unsigned long long x[kChains], pa, pb;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(pa) : "f"(a));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(pb) : "f"(b));
+#pragma unroll
+    for (int i = 0; i < kChains; ++i) asm("mov.b64 %0, {%1, %2};" : "=l"(x[i]) : "f"((float)(threadIdx.x + i)), "f"((float)i));
+    for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+        for (int i = 0; i < kChains; ++i) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(x[i]) : "l"(pa), "l"(pb));
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < kChains; ++i) {
+        float lo, hi;
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(x[i]));
+        s += lo + hi;
+    }
+    if (s == 12345.678f) out[0] = s;
+}
+
 }  // namespace
 
-extern "C" int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, void* stream) {
-    if (!fma_tflops || !add_tinst) return RICK_EINVAL;
+extern "C" int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, double* fma2_tflops, void* stream) {
+    if (!fma_tflops || !add_tinst || !fma2_tflops) return RICK_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, sms = 0;
     RICK_CUDA(cudaGetDevice(&dev));
@@ -38,12 +59,13 @@ extern "C" int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, voi
     RICK_CUDA(cudaEventCreate(&e1));
     const int blocks = sms * 8, n_iter = 8192;
     const double ops = (double)blocks * 256.0 * (double)n_iter * (double)kChains;
-    double best[2] = {0.0, 0.0};
-    for (int kind = 0; kind < 2; ++kind) {
+    double best[3] = {0.0, 0.0, 0.0};
+    for (int kind = 0; kind < 3; ++kind) {
         for (int rep = 0; rep < 4; ++rep) {      // first repetition warms up
             RICK_CUDA(cudaEventRecord(e0, st));
             if (kind == 0) k_fp32_rate<true><<<blocks, 256, 0, st>>>(out, n_iter, 0.999f, 0.001f);
-            else k_fp32_rate<false><<<blocks, 256, 0, st>>>(out, n_iter, 0.999f, 0.001f);
+            else if (kind == 1) k_fp32_rate<false><<<blocks, 256, 0, st>>>(out, n_iter, 0.999f, 0.001f);
+            else k_fp32x2_rate<<<blocks, 256, 0, st>>>(out, n_iter, 0.999f, 0.001f);
             RICK_CUDA(cudaEventRecord(e1, st));
             RICK_CUDA(cudaEventSynchronize(e1));
             float ms = 0.f;
@@ -58,5 +80,6 @@ extern "C" int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, voi
     RICK_LAUNCH_CHECK();
     *fma_tflops = 2.0 * best[0];      // 2 flop per fused multiply-add
     *add_tinst = best[1];             // 1e12 fp32 add instructions (lane-ops) per second
+    *fma2_tflops = 4.0 * best[2];     // packed: 2 fused multiply-adds = 4 flop per lane-op
     return RICK_OK;
 }

@@ -458,6 +458,18 @@ int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_by
         if (rc == RICK_OK) rc = rick_rowfft_impl(p, grid, st);
         return rc;
     }
+    if (p->fused == 2 && p->split && rick_rowbig_supported(p)) {
+        // own row kernel on the defined rows only (rowbig.cu), then sweep A, which reads only those rows
+        StageTimer tm(p, RICK_T_FFT, st);
+        int rc = rick_rows_list_all(p, st);
+        {
+            StageTimer tr(p, RICK_T_FFT_ROWS, st);
+            if (rc == RICK_OK) rc = rick_rowbig_impl(p, grid, st);
+        }
+        StageTimer ta(p, RICK_T_FFT_COL_A, st);
+        if (rc == RICK_OK) rc = rick_colsplit_a_impl(p, grid, st);
+        return rc;
+    }
     if (p->fused) {   // rows only (+ sweep A of the split engine); rick_wcorrect_accumulate finishes the transform
         if (p->fft_rows_work_bytes > 0 && (!fft_work || fft_work_bytes < p->fft_rows_work_bytes)) return RICK_ENOMEM;
         if (cufftSetStream(p->fft_rows, st) != CUFFT_SUCCESS) return RICK_ECUFFT;

@@ -457,6 +457,8 @@ def test_fusion_mode_2_row_occupancy(name, M, plan, kernel):
     ("100M", 300_000, dict(N=2048, Nw=4), "c128", 2),         # 32 x 64
     ("100M", 400_000, dict(N=4096, Nw=4), "c128", 2),         # 64 x 64: the 100M plan's transform
     ("500M", 400_000, dict(N=4096, Nw=4), "c64", 1),          # 64 x 64
+    ("500M", 400_000, dict(N=4096, Nw=3), "c64", 2),          # own row kernel (rowbig.cu) 64 x 64, fp32
+    ("100M", 300_000, dict(N=8192, Nw=2), "c128", 2),         # own row kernel 64 x 128, fp64
     ("500M", 400_000, dict(N=8192, Nw=3), "c64", 2),          # 64 x 128: the 500M plan's transform, odd plane count
     ("hotspot", 400_001, dict(N=16384, Nw=2), "c64", 2),      # 128 x 128: the hotspot plan's transform, support 9
 ])
