@@ -16,6 +16,7 @@
 // (3.7e-7 rad at worst) and reduced to [-1/2, 1/2), then the hardware sine / cosine in fp32 on the reduced
 // argument (abs error < 5e-7, the precision of the fp32 planes themselves); the product in fp32, the plane
 // sum in fp64.
+#include "fft_radix.cuh"
 #include "rick_internal.cuh"
 
 namespace {
@@ -29,65 +30,10 @@ constexpr int kPadShift = 5;     // 4 float2 of padding after every 32 float2 (b
 template <int X = 0>
 __device__ __forceinline__ constexpr int padded(int idx) { return idx + ((idx >> kPadShift) << 2) + (idx >> 9) * X; }
 
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-
-// 4-point inverse DFT (omega_4 = +i), in place
-__device__ __forceinline__ void dft4(float2& a, float2& b, float2& c, float2& d) {
-    const float2 s0 = make_float2(a.x + c.x, a.y + c.y), d0 = make_float2(a.x - c.x, a.y - c.y);
-    const float2 s1 = make_float2(b.x + d.x, b.y + d.y), d1 = make_float2(b.x - d.x, b.y - d.y);
-    a = make_float2(s0.x + s1.x, s0.y + s1.y);
-    c = make_float2(s0.x - s1.x, s0.y - s1.y);
-    b = make_float2(d0.x - d1.y, d0.y + d1.x);      // d0 + i d1
-    d = make_float2(d0.x + d1.y, d0.y - d1.x);      // d0 - i d1
-}
-
-// R-point inverse DFT, y_u = sum_t x_t exp(+2 pi i u t / R), natural order in and out
-template <int R> __device__ __forceinline__ void dft(float2* v);
-template <> __device__ __forceinline__ void dft<1>(float2*) {}
-template <> __device__ __forceinline__ void dft<2>(float2* v) {
-    const float2 a = v[0], b = v[1];
-    v[0] = make_float2(a.x + b.x, a.y + b.y);
-    v[1] = make_float2(a.x - b.x, a.y - b.y);
-}
-template <> __device__ __forceinline__ void dft<4>(float2* v) { dft4(v[0], v[1], v[2], v[3]); }
-template <> __device__ __forceinline__ void dft<8>(float2* v) {
-    float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
-    dft4(e0, e1, e2, e3);
-    dft4(o0, o1, o2, o3);
-    const float r = 0.70710678118654752f;
-    const float2 t1 = make_float2(r * (o1.x - o1.y), r * (o1.x + o1.y));     // o1 * exp(+i pi/4)
-    const float2 t2 = make_float2(-o2.y, o2.x);                               // o2 * i
-    const float2 t3 = make_float2(-r * (o3.x + o3.y), r * (o3.x - o3.y));    // o3 * exp(+3 i pi/4)
-    v[0] = make_float2(e0.x + o0.x, e0.y + o0.y); v[4] = make_float2(e0.x - o0.x, e0.y - o0.y);
-    v[1] = make_float2(e1.x + t1.x, e1.y + t1.y); v[5] = make_float2(e1.x - t1.x, e1.y - t1.y);
-    v[2] = make_float2(e2.x + t2.x, e2.y + t2.y); v[6] = make_float2(e2.x - t2.x, e2.y - t2.y);
-    v[3] = make_float2(e3.x + t3.x, e3.y + t3.y); v[7] = make_float2(e3.x - t3.x, e3.y - t3.y);
-}
-// 16 = 4 x 4: t = 4a + b, u = c + 4d:  w16^(ut) = w4^(ac) w16^(bc) w4^(bd)
-template <> __device__ __forceinline__ void dft<16>(float2* v) {
-#pragma unroll
-    for (int b = 0; b < 4; ++b) dft4(v[b], v[4 + b], v[8 + b], v[12 + b]);   // over a: result c at v[4c + b]
-    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, r = 0.70710678118654752f;
-    const float2 w1 = make_float2(c1, s1), w2 = make_float2(r, r), w3 = make_float2(s1, c1);
-    const float2 w6 = make_float2(-r, r), w9 = make_float2(-c1, -s1);
-    // z(b,c) at v[4c + b] *= w16^(bc)
-    v[4 + 1] = cmul(v[4 + 1], w1); v[4 + 2] = cmul(v[4 + 2], w2); v[4 + 3] = cmul(v[4 + 3], w3);
-    v[8 + 1] = cmul(v[8 + 1], w2); v[8 + 2] = make_float2(-v[8 + 2].y, v[8 + 2].x); v[8 + 3] = cmul(v[8 + 3], w6);
-    v[12 + 1] = cmul(v[12 + 1], w3); v[12 + 2] = cmul(v[12 + 2], w6); v[12 + 3] = cmul(v[12 + 3], w9);
-#pragma unroll
-    for (int c = 0; c < 4; ++c) dft4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);   // over b: d at v[4c + d]
-    // y(c + 4d) sits at v[4c + d]: transpose the 4 x 4 so that y_u is at v[u]
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int d = c + 1; d < 4; ++d) {
-            const float2 t = v[4 * c + d];
-            v[4 * c + d] = v[4 * d + c];
-            v[4 * d + c] = t;
-        }
-}
+// complex product and the small inverse DFTs (natural order in and out) in the packed fp32 arithmetic of
+// fft_radix.cuh (add / mul / fma .f32x2: one issue slot per (re, im) pair)
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return cx_mul<float2>(a, b); }
+template <int R> __device__ __forceinline__ void dft(float2* v) { cx_dft<R, float2>(v); }
 
 // One in-place decimation-in-frequency pass of radix R over sub-transforms of length n = 2^LOG2n of the
 // N = 2^LOG2N point columns:  for every sub-block B, offset m < n/R, column c:
@@ -234,8 +180,7 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         const int idx = owned_slot(e);
         const int q = slot_to_freq(idx / kC, N), p = p0 + (idx % kC);
         const double l = (double)(p - N / 2) * g.dl, m = (double)(q - N / 2) * g.dl;
-        const double r2 = l * l + m * m;
-        nm1r[e] = -r2 / (1.0 + sqrt(1.0 - r2));
+        nm1r[e] = rick_nm1_fast(l * l + m * m);
         acc[e] = 0.0;
     }
     auto screen_add = [&](int e, float2 v, double wk) {

@@ -191,22 +191,8 @@ template <int E> struct Screen<double, E> {
     }
 };
 
-// n - 1 = -(l^2 + m^2) / (1 + sqrt(1 - l^2 - m^2)) without the library's IEEE square root and division (two
-// subroutine calls per output): fp32 seeds refined by two Newton steps each in fp64 (error < 2 ulp; a thread
-// needs E of these before its first plane, which weighed 14 % of the kernel at 16 planes)
-RICK_DI double nm1_fast(double r2) {
-    const double y = 1.0 - r2;
-    double x = (double)rsqrtf((float)y);
-    x = x * fma(-0.5 * y, x * x, 1.5);
-    x = x * fma(-0.5 * y, x * x, 1.5);
-    const double d = fma(y, x, 1.0);                     // 1 + sqrt(y)
-    double r = (double)__frcp_rn((float)d);
-    r = r * fma(-d, r, 2.0);
-    r = r * fma(-d, r, 2.0);
-    return -r2 * r;
-}
 template <typename real> RICK_DI double nm1_of(double r2);
-template <> RICK_DI double nm1_of<float>(double r2) { return nm1_fast(r2); }
+template <> RICK_DI double nm1_of<float>(double r2) { return rick_nm1_fast(r2); }
 template <> RICK_DI double nm1_of<double>(double r2) { return -r2 / (1.0 + sqrt(1.0 - r2)); }
 
 template <typename C2, int L> struct ColB {

@@ -23,6 +23,7 @@
 // signs are compile-time negations of the taps, the run-constant remainder is the sign of the weight.
 #include <string.h>
 
+#include "fft_radix.cuh"
 #include "rick_internal.cuh"
 
 namespace {
@@ -337,11 +338,12 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 #pragma unroll
     for (int pass = 0; pass < kPasses; ++pass) {
         const int b0 = pass * RB;
-        float ar[RB][W], ai[RB][W];
+        // (re, im) of a cell in one register pair: the accumulation is one packed fma.rn.f32x2 (FFMA2) per cell
+        float2 acc[RB][W];
 #pragma unroll
         for (int r = 0; r < RB; ++r)
 #pragma unroll
-            for (int a = 0; a < W; ++a) ar[r][a] = ai[r][a] = 0.f;
+            for (int a = 0; a < W; ++a) acc[r][a] = make_float2(0.f, 0.f);
         uint32_t cij = 0xFFFFFFFFu, ck = 0;
 
         auto flush = [&]() {
@@ -362,7 +364,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
                     if (b0 + r < S) {
 #pragma unroll
                         for (int a = 0; a < W; a += 2)
-                            red_add_pair(rowp[r] + a, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
+                            red_add_pair(rowp[r] + a, acc[r][a].x, acc[r][a].y, acc[r][a + 1].x, acc[r][a + 1].y);
                     }
             } else {
 #pragma unroll
@@ -370,15 +372,15 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
                     if (b0 + r < S) {
 #pragma unroll
                         for (int a = 0; a < W; a += 2) {
-                            if (a + 2 == W) red_add_cell(rowp[r] + a, ar[r][a], ai[r][a]);
-                            else red_add_pair(rowp[r] + a, ar[r][a], ai[r][a], ar[r][a + 1], ai[r][a + 1]);
+                            if (a + 2 == W) red_add_cell(rowp[r] + a, acc[r][a].x, acc[r][a].y);
+                            else red_add_pair(rowp[r] + a, acc[r][a].x, acc[r][a].y, acc[r][a + 1].x, acc[r][a + 1].y);
                         }
                     }
             }
 #pragma unroll
             for (int r = 0; r < RB; ++r)
 #pragma unroll
-                for (int a = 0; a < W; ++a) ar[r][a] = ai[r][a] = 0.f;
+                for (int a = 0; a < W; ++a) acc[r][a] = make_float2(0.f, 0.f);
         };
 
         auto one = [&](uint32_t ij, uint32_t k, float dx, float dy, float vr, float vi) {
@@ -412,12 +414,9 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
 #pragma unroll
             for (int r = 0; r < RB; ++r) {
                 if (b0 + r < S) {
-                    const float yr = gy[b0 + r] * vr, yi = gy[b0 + r] * vi;
+                    const float2 y = cx_scale(gy[b0 + r], make_float2(vr, vi));
 #pragma unroll
-                    for (int a = 0; a < W; ++a) {
-                        ar[r][a] = fmaf(gx[a], yr, ar[r][a]);
-                        ai[r][a] = fmaf(gx[a], yi, ai[r][a]);
-                    }
+                    for (int a = 0; a < W; ++a) acc[r][a] = cx_fma_real(gx[a], y, acc[r][a]);
                 }
             }
         };
@@ -528,7 +527,7 @@ int rick_grid_impl(rick_plan* p, void* grid, cudaStream_t st) {
     switch (p->g.S) {
         case 3:  if (f64) launch_runs<double, 3, 3>(p, grid, st);  else rc = launch_rec<3, 3>(p, grid, st); break;
         case 5:  if (f64) launch_runs<double, 5, 5>(p, grid, st);  else rc = launch_rec<5, 5>(p, grid, st); break;
-        case 7:  if (f64) launch_runs<double, 7, 4>(p, grid, st);  else rc = launch_rec<7, 7>(p, grid, st); break;
+        case 7:  if (f64) launch_runs<double, 7, 7>(p, grid, st);  else rc = launch_rec<7, 7>(p, grid, st); break;
         case 9:  if (f64) launch_runs<double, 9, 3>(p, grid, st);  else rc = launch_rec<9, 9>(p, grid, st); break;
         case 11: if (f64) launch_runs<double, 11, 2>(p, grid, st); else rc = launch_rec<11, 4>(p, grid, st); break;
         case 13: if (f64) launch_runs<double, 13, 2>(p, grid, st); else rc = launch_rec<13, 3>(p, grid, st); break;

@@ -155,6 +155,21 @@ __device__ __forceinline__ uint32_t rick_tile_of_sort_key(const RickGeom& g, uin
     return sk == g.sort_sentinel ? g.n_bins : (sk >> g.cell_bits);
 }
 
+// n - 1 = -(l^2 + m^2) / (1 + sqrt(1 - l^2 - m^2)) without the library's IEEE square root and division (two
+// subroutine calls per output): fp32 seeds refined by two Newton steps each in fp64 (error < 2 ulp).  Used by the
+// fp32-mesh column kernels, whose threads need 16 of these before their first plane.
+__device__ __forceinline__ double rick_nm1_fast(double r2) {
+    const double y = 1.0 - r2;
+    double x = (double)rsqrtf((float)y);
+    x = x * fma(-0.5 * y, x * x, 1.5);
+    x = x * fma(-0.5 * y, x * x, 1.5);
+    const double d = fma(y, x, 1.0);                     // 1 + sqrt(y)
+    double r = (double)__frcp_rn((float)d);
+    r = r * fma(-d, r, 2.0);
+    r = r * fma(-d, r, 2.0);
+    return -r2 * r;
+}
+
 // translation-unit entry points (host side)
 void rick_stage_begin(rick_plan* p, int stage, cudaStream_t st);
 void rick_stage_end(rick_plan* p, int stage, cudaStream_t st);

@@ -74,16 +74,22 @@ k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* 
     for (int s = 0; s < Ra2; ++s) pw[s] = tw_g[(j2 * Ra1 * s) & (N - 1)];
     __syncthreads();
 
-    for (int r = blockIdx.x; r < n; r += gridDim.x) {
-        C2* x = planes + (size_t)list[r] * N;
-        C2 v[32];
-        // ---- step 1, pass 1: radix Ra1 over j1 = m + t Ra2, from global memory
+    // the inputs of the first pass (radix Ra1 over j1 = m + t Ra2) come straight from global memory; the next row's
+    // are requested as soon as this row's last butterflies have left the registers, before the closing barrier
+    C2 v[32];
+    auto fetch = [&](int r) {
+        const C2* x = planes + (size_t)__ldg(list + r) * N;
 #pragma unroll
         for (int i = 0; i < 32 / Ra1; ++i) {
             const int m = a0 + i * aStep;
 #pragma unroll
             for (int t = 0; t < Ra1; ++t) v[i * Ra1 + t] = ldg_stream(x + (m + t * Ra2) * N2 + j2);
         }
+    };
+    fetch(blockIdx.x);
+    for (int r = blockIdx.x; r < n; r += gridDim.x) {
+        C2* x = planes + (size_t)list[r] * N;
+        // ---- step 1, pass 1
 #pragma unroll
         for (int i = 0; i < 32 / Ra1; ++i) {
             const int m = a0 + i * aStep;
@@ -134,6 +140,7 @@ k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* 
 #pragma unroll
             for (int s = 0; s < Rb2; ++s) x[q1 + N1 * (u + Rb1 * s)] = v[i * Rb2 + s];
         }
+        if (r + (int)gridDim.x < n) fetch(r + (int)gridDim.x);
         __syncthreads();                         // the buffer is free for the next row
     }
 }

@@ -354,13 +354,17 @@ def test_fused_column_transform(name, M, plan):
     tw = np.outer(t, t) / t[N // 2] ** 2
     assert (np.abs(twice - 2 * img) * tw).max() <= 2e-6 * np.abs(img * tw).max()
     im.close()
-    # a c128 plan or an unsupported size refuses fusion and stays on the two-kernel path
-    im2 = B.Imager(dtype="c128", M_max=16, fused=True, **pa)
+    # a c128 plan takes the split column transform (colsplit.cu); a mesh size that is not a power of two refuses
+    # fusion and stays on the two-kernel path
+    im2 = B.Imager(dtype="c128", M_max=16, fused=True, alloc_mesh=False, **pa)
+    assert im2.fused
+    im2.close()
+    im2 = B.Imager(dtype="c64", M_max=16, fused=True, alloc_mesh=False, **dict(pa, N=480, dl=pa["dl"] * N / 480))
     assert not im2.fused
     im2.close()
     # so does a plan whose |w| reaches 2^28 wavelengths (the fused screen's fixed-point phase fraction)
     pa3 = dict(pa, w_min=-1.0, w_max=float(2 ** 28))
-    im3 = B.Imager(dtype="c64", M_max=16, fused=True, **pa3)
+    im3 = B.Imager(dtype="c64", M_max=16, fused=True, alloc_mesh=False, **pa3)
     assert not im3.fused
     im3.close()
 
