@@ -302,13 +302,17 @@ def main():
         fft_rows_b = 2 * live_bytes if own_rows else 2 * mesh_bytes      # else batched library transforms of every row
         col_a_b = live_bytes + mesh_bytes    # sweep A reads the defined rows, writes every row
         fft_b, wc_b = fft_rows_b + col_a_b, mesh_bytes + cfg.N * cfg.N * 8
+    indirect = cfg.dtype == "c64"       # fp32 mesh: rick_bin gathers nothing; the gridder fetches 32-B records by index
     alg = {   # algorithmic bytes per stage
         "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
         # sort: first pass 4 r + 8 w, middle passes 8 r + 8 w, last pass 8 r and, fused into it, the gather
         # (one 32-B record in, sorted SoA 24 B + gridder records 24 B out per kept visibility)
-        "sort": ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept,
+        # (indirect: every pass after the first is 8 r + 8 w and nothing is gathered; the gridder reads 4 B of index
+        # and one 32-B record per kept visibility)
+        "sort": ((12 + 16 * (n_pass - 1)) * M if indirect else
+                 ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept),
         "zero": live_bytes if im.fused == 2 else mesh_bytes,
-        "grid": 24 * n_kept,
+        "grid": (4 + 32) * n_kept if indirect else 24 * n_kept,
         "fft": fft_b, "fft_rows": fft_rows_b, "fft_col_a": col_a_b,
         "wcorrect": wc_b,
     }
@@ -401,7 +405,7 @@ def main():
         "vs_baseline": None, "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
         "config": {"workload": args.config + (" (profiling subset)" if args.M or args.Nw else ""), "M": M, "M_kept": n_kept, "sort_passes": n_pass, "N": cfg.N, "Nw": cfg.Nw,
                    "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype,
-                   "fusion_mode": int(im.fused),
+                   "fusion_mode": int(im.fused), "rick_bin_sorted_outputs": bool(im.sorted_outputs),
                    "column_engine": "split (colsplit.cu)" if split else ("one sweep (colfft.cu)" if one_sweep else "cuFFT 2-D + K5"),
                    "mesh_rows_defined": rows_defined, "mesh_rows": rows_total,
                    "parallelism": "replicas only" if world > 1 else "single GPU",

@@ -122,11 +122,17 @@ int rick_plan_sort_layout(const rick_plan* plan, int* key_bits, int* n_pass, int
  *   M                     number of visibilities, 0 <= M < 2^32 - 1
  *   u, v, w               device float[M], baseline coordinates in wavelengths
  *   vis                   device float2[M] (complex64), weight: device float[M]
- *   u_s .. weight_s       device outputs of capacity M: the kept visibilities in the stable order
- *                         (key, input index); only the first n_kept entries are written
+ *   u_s .. weight_s       device outputs of capacity M: the kept visibilities in the stable order [D4'];
+ *                         only the first n_kept entries are written.  Either all five, or all five NULL
+ *                         (RICK_C64 plans only): then nothing is gathered -- the library keeps the sorted
+ *                         input indices in the workspace and rick_grid fetches its 32-byte records through
+ *                         them ("indirect mode": the random reads of the gather run under the gridder's
+ *                         arithmetic instead of under a sort pass).  RICK_C128 plans need the five outputs
+ *                         (the fp64 gridder reads them): RICK_EINVAL otherwise
  *   key_out               nullable device unsigned[M]: key of every input visibility,
  *                         key = (k T + (j0 >> 5)) T + (i0 >> 5), T = N/32; dropped -> Nw T^2
- *   perm_out              nullable device unsigned[M]: sorted rank -> input index (all M, sentinels last)
+ *   perm_out              nullable device unsigned[M]: sorted rank -> input index (all M, dropped ones last; in
+ *                         indirect mode a copy of the index the gridder uses)
  *   bin_start_out         nullable device unsigned long long[Nw T^2 + 2]: number of visibilities with
  *                         key < b (entry Nw T^2 is n_kept, the last entry is M)
  *   workspace             device scratch of at least rick_plan_workspace_bytes(M) bytes, 256-byte aligned

@@ -165,10 +165,12 @@ def rick_plan_destroy(plan: int) -> None:
 def rick_bin(plan: int, M: int, u, v, w, vis, weight, u_s, v_s, w_s, vis_s, weight_s, workspace, n_kept,
              key_out=None, perm_out=None, bin_start_out=None, stream=None) -> None:
     f32, c64 = torch.float32, torch.complex64
-    for t, dt, nm in ((u, f32, "u"), (v, f32, "v"), (w, f32, "w"), (vis, c64, "vis"), (weight, f32, "weight"),
-                      (u_s, f32, "u_s"), (v_s, f32, "v_s"), (w_s, f32, "w_s"), (vis_s, c64, "vis_s"),
-                      (weight_s, f32, "weight_s")):
+    for t, dt, nm in ((u, f32, "u"), (v, f32, "v"), (w, f32, "w"), (vis, c64, "vis"), (weight, f32, "weight")):
         _dev(t, dt, M, nm)
+    for t, dt, nm in ((u_s, f32, "u_s"), (v_s, f32, "v_s"), (w_s, f32, "w_s"), (vis_s, c64, "vis_s"),
+                      (weight_s, f32, "weight_s")):
+        if t is not None:        # all five None: no sorted copies (fp32 mesh; the gridder fetches records by index)
+            _dev(t, dt, M, nm)
     _dev(workspace, torch.uint8, None, "workspace")
     _dev(n_kept, torch.int64, 1, "n_kept")
     if key_out is not None:
@@ -233,7 +235,8 @@ class Imager:
 
     def __init__(self, N: int, Nw: int, support: int, sigma: float, w_min: float, w_max: float, dl: float,
                  dtype: str = "c64", M_max: int = 0, device="cuda", fused: int = 0,
-                 kernel: str = "gauss", beta: float = 0.0, alloc_mesh: bool = True):
+                 kernel: str = "gauss", beta: float = 0.0, alloc_mesh: bool = True,
+                 sorted_outputs: Optional[bool] = None):
         if not torch.cuda.is_available():
             raise RickError("librick_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -248,6 +251,11 @@ class Imager:
                 rick_plan_set_kernel(self.plan, RICK_KERNEL_KB, beta)
             elif kernel != "gauss":
                 raise RickError(f"unknown gridding kernel {kernel!r}")
+        # sorted SoA copies of the kept visibilities (an output of rick_bin): the fp64 gridder reads them; on the
+        # fp32 mesh they are optional, and without them rick_bin gathers nothing (indirect mode, rick_b200.h)
+        self.sorted_outputs = (dtype == "c128") if sorted_outputs is None else bool(sorted_outputs)
+        if dtype == "c128" and not self.sorted_outputs:
+            raise RickError("the fp64 mesh needs the sorted outputs of rick_bin")
         self.M_max = 0
         # alloc_mesh = False: a binning-only helper (rick_bin needs neither the mesh nor the image)
         self.grid = torch.empty((Nw, N, N) if alloc_mesh else (0,), dtype=self.cdtype, device=self.device)
@@ -265,9 +273,10 @@ class Imager:
             return
         m = max(int(M), 1)
         d = self.device
-        self.sorted = dict(u=torch.empty(m, dtype=torch.float32, device=d), v=torch.empty(m, dtype=torch.float32, device=d),
-                           w=torch.empty(m, dtype=torch.float32, device=d), vis=torch.empty(m, dtype=torch.complex64, device=d),
-                           weight=torch.empty(m, dtype=torch.float32, device=d))
+        ms = m if self.sorted_outputs else 0
+        self.sorted = dict(u=torch.empty(ms, dtype=torch.float32, device=d), v=torch.empty(ms, dtype=torch.float32, device=d),
+                           w=torch.empty(ms, dtype=torch.float32, device=d), vis=torch.empty(ms, dtype=torch.complex64, device=d),
+                           weight=torch.empty(ms, dtype=torch.float32, device=d))
         bin_bytes, _ = rick_plan_workspace_bytes(self.plan, m)
         self.workspace = torch.empty(bin_bytes, dtype=torch.uint8, device=d)
         self.staging = None
@@ -288,7 +297,7 @@ class Imager:
     def bin(self, u, v, w, vis, weight, key_out=None, perm_out=None, bin_start_out=None) -> None:
         M = int(u.numel())
         self.reserve(M)
-        s = self.sorted
+        s = self.sorted if self.sorted_outputs else dict(u=None, v=None, w=None, vis=None, weight=None)
         rick_bin(self.plan, M, u, v, w, vis, weight, s["u"], s["v"], s["w"], s["vis"], s["weight"], self.workspace,
                  self.n_kept, key_out=key_out, perm_out=perm_out, bin_start_out=bin_start_out)
 
@@ -323,7 +332,8 @@ class Imager:
         for t in (u, v, w, vis, weight, image_host):
             if t.is_cuda or not t.is_contiguous():
                 raise RickError("run_from_host: host tensors expected")
-        g, s = self.staging, self.sorted
+        g = self.staging
+        s = self.sorted if self.sorted_outputs else dict(u=None, v=None, w=None, vis=None, weight=None)
         b = _DeviceBuffers(
             _ptr(g["u"]), _ptr(g["v"]), _ptr(g["w"]), _ptr(g["vis"]), _ptr(g["weight"]),
             _ptr(s["u"]), _ptr(s["v"]), _ptr(s["w"]), _ptr(s["vis"]), _ptr(s["weight"]),

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
                                                 const float2* __restrict__ vis, const float* __restrict__ wt,
                                                 uint32_t* __restrict__ key, float4* __restrict__ rec,
                                                 uint32_t* __restrict__ tile_key_out, uint32_t* __restrict__ hist,
-                                                unsigned long long* __restrict__ n_kept, SortLayout lay) {
+                                                unsigned long long* __restrict__ n_kept, SortLayout lay, int rec_form) {
     __shared__ uint32_t sh[RICK_MAX_PASSES][kRadix];
     for (int i = threadIdx.x; i < RICK_MAX_PASSES * kRadix; i += blockDim.x) (&sh[0][0])[i] = 0;
     __syncthreads();
@@ -107,8 +107,15 @@ __global__ void __launch_bounds__(256) k_keygen(RickGeom g, long long M, const f
             kk = keep ? rick_sort_key(g, r) : g.sort_sentinel;
             kept += keep ? 1u : 0u;
             key[m] = kk;
-            rec[2 * m] = make_float4(uu, vv, ww, vi.x);
-            rec[2 * m + 1] = make_float4(vi.y, wgt, 0.f, 0.f);
+            if (rec_form == 0) {     // raw visibility: the gather copies it to the sorted SoA and derives the gridder record
+                rec[2 * m] = make_float4(uu, vv, ww, vi.x);
+                rec[2 * m + 1] = make_float4(vi.y, wgt, 0.f, 0.f);
+            } else {                 // the gridder record itself (rick_internal.cuh): the fp32 gridder fetches it by index
+                const float ws = ((r.j0 - g.h) & 1) ? -wgt : wgt;
+                rec[2 * m] = make_float4(__uint_as_float((uint32_t)r.i0 | ((uint32_t)r.j0 << 16)), __uint_as_float((uint32_t)r.k),
+                                         (float)((double)r.i0 - r.x), (float)((double)r.j0 - r.y));
+                rec[2 * m + 1] = make_float4(ws * vi.x, ws * vi.y, 0.f, 0.f);
+            }
             if (tile_key_out) tile_key_out[m] = keep ? rick_tile_key(g, r) : g.n_bins;
         }
         // digit histograms: lanes that share lane 0's digit (the common case in the skewed high
@@ -462,6 +469,14 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
     const RickGeom& g = p->g;
     Workspace ws = carve(workspace, M);
     p->bound = false;
+    // No sorted SoA asked for (fp32 mesh only): nothing is gathered.  The staging records are the gridder records,
+    // the sort ends with the sorted (key, index) pairs, and the gridder fetches its records through the index
+    // -- the 1e9 random 32-byte reads of the gather (the GPU's random-access rate bounds them) then run under the
+    // gridder's arithmetic instead of under a sort pass that has none.
+    const bool indirect = (u_s == nullptr);
+    p->indirect = indirect;
+    p->gidx = nullptr;
+    p->grec = nullptr;
     RICK_CUDA(cudaMemsetAsync(n_kept_dev, 0, sizeof(long long), st));
     if (M == 0) {
         if (bin_start_out) {
@@ -481,7 +496,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             const long long cap = (long long)p->sm_count * 16;
             const int blocks = (int)(want < 1 ? 1 : (want > cap ? cap : want));
             k_keygen<<<blocks, 256, 0, st>>>(g, M, u, v, w, vis, weight, ws.key_a, ws.rec, key_out, ws.hist,
-                                             (unsigned long long*)n_kept_dev, lay);
+                                             (unsigned long long*)n_kept_dev, lay, indirect ? 1 : 0);
             RICK_LAUNCH_CHECK();
             p->launches++;
         }
@@ -495,7 +510,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         uint32_t *kin = ws.key_a, *iin = ws.idx_a, *kout = ws.key_b, *iout = ws.idx_b;
         (void)iout;
         // the gather rides in the last pass unless the caller wants the sorted (key, index) arrays
-        const bool fuse_gather = !perm_out && !bin_start_out;
+        const bool fuse_gather = !indirect && !perm_out && !bin_start_out;
         GatherOut go;
         go.g = g; go.rec = ws.rec;
         go.u_s = u_s; go.v_s = v_s; go.w_s = w_s; go.vis_s = vis_s; go.wt_s = weight_s;
@@ -523,6 +538,19 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         rick_stage_begin(p, RICK_T_GATHER, st);
         if (fuse_gather) {
             p->grec_a = (const uint2*)kout;
+        } else if (indirect) {
+            // sorted (key, index) live in kin / iin; kept visibilities come first
+            if (perm_out) RICK_CUDA(cudaMemcpyAsync(perm_out, iin, 4 * (size_t)M, cudaMemcpyDeviceToDevice, st));
+            if (bin_start_out) {
+                const long long want = (M + 1 + 255) / 256;
+                const long long cap = (long long)p->sm_count * 16;
+                k_bin_start<<<(int)(want > cap ? cap : want), 256, 0, st>>>(g, M, kin, bin_start_out);
+                RICK_LAUNCH_CHECK();
+                p->launches++;
+            }
+            p->gidx = iin;
+            p->gkey = kin;
+            p->grec = ws.rec;
         } else {
             // sorted (key, index) now live in kin / iin
             if (perm_out) {
@@ -545,6 +573,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
         }
         rick_stage_end(p, RICK_T_GATHER, st);
     }
+    if (M == 0) p->indirect = false;
     if (p->fused == 2) {
         p->n_kept_dev = n_kept_dev;
         const int rc = rick_rows_mark(p, M, st);

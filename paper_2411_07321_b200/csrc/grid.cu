@@ -296,18 +296,41 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 
-template <int S, int RB, int L, int NBUF, int KIND>
+// pieces of a record fetched at random (indirect mode): ask L2 for 64 bytes, not the whole 128-byte line
+// (hotspot gridder 40.2 -> 37.7 ms: the random reads share the DRAM with the reductions' read-modify-writes)
+__device__ __forceinline__ void cp_async16_rand(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global.L2::64B [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async8_rand(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global.L2::64B [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+// kIdx = false: the three sorted record streams ga / gb / gc (written by rick_bin's gather).
+// kIdx = true (indirect mode, rick_bin without sorted SoA outputs): the record of the sorted visibility at
+// position i is the 32-byte staging record grec[gidx[i]] in INPUT order.  A stage's indices are copied to shared
+// memory one stage ahead (coalesced 16-byte cp.async), then every record is fetched with one 16-byte and one
+// 8-byte cp.async -- 2 x 128 x L random sector reads in flight per SM while the stage before is accumulated.
+// The gather of the sort (bound by the GPU's random-access rate) disappears into this kernel.
+template <int S, int RB, int L, int NBUF, int KIND, bool kIdx>
 __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst tc, const long long* __restrict__ n_kept,
                                                          const uint2* __restrict__ ga, const float2* __restrict__ gb,
-                                                         const float2* __restrict__ gc, float2* __restrict__ grid,
+                                                         const float2* __restrict__ gc, const uint32_t* __restrict__ gidx,
+                                                         const float4* __restrict__ grec, float2* __restrict__ grid,
                                                          int n_stage, KbPoly kp) {
     constexpr int h = (S - 1) / 2;
     constexpr int kPasses = (S + RB - 1) / RB;
     constexpr int W = S + 1;                    // even-aligned window, see k_grid_runs
     constexpr int PPT = L / 2;                  // 16-byte pieces (two records) per thread, stream and stage
     constexpr int NP = kRunThreads * PPT;       // pieces per stream and stage
-    static_assert(PPT >= 8 && (PPT & (PPT - 1)) == 0, "L must be a power of two >= 16");
-    extern __shared__ uint4 stage[];            // [2 buffers][3 streams][NP]
+    static_assert((L & (L - 1)) == 0 && L >= (kIdx ? 8 : 16), "L: a power of two, >= 16 (>= 8 in indirect mode)");
+    extern __shared__ uint4 stage[];            // direct: [2 buffers][3 streams][NP]; indirect: see below
+    // indirect layout: A[2][128 L] uint4 (cell, plane, offsets), B[2][128 L] uint2 (weight * V), idx[2][128 L] u32
+    constexpr int NR = kRunThreads * L;         // records per stage
+    uint4* recA = stage;
+    uint2* recB = reinterpret_cast<uint2*>(stage + 2 * NR);
+    uint32_t* idxb = reinterpret_cast<uint32_t*>(recB + 2 * NR);
     const long long n = *n_kept;
     const long long per_thread = (long long)L * n_stage;
     const long long cta_first = (long long)blockIdx.x * (kRunThreads * per_thread);
@@ -333,6 +356,29 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    // indirect mode: the thread's own L indices of stage st (contiguous), and the records of stage st
+    auto issue_idx = [&](int st) {
+        const long long pos = first + (long long)st * L;
+        if (pos < n) {
+            uint32_t* dst = idxb + (st & 1) * NR + tid * L;
+#pragma unroll
+            for (int x = 0; x < L; x += 4) cp_async16(dst + x, gidx + pos + x);
+        }
+    };
+    auto issue_rec = [&](int st) {
+        const uint32_t* ib = idxb + (st & 1) * NR;
+#pragma unroll 4
+        for (int q = tid; q < NR; q += kRunThreads) {
+            const int t = q / L, r = q % L;
+            const long long pos = cta_first + (long long)t * per_thread + (long long)st * L + r;
+            if (pos < n) {
+                const float4* src = grec + 2 * (size_t)ib[q];
+                // swizzles: a quarter warp's 16-byte reads (a half warp's 8-byte reads) of one r hit distinct banks
+                cp_async16_rand(recA + (st & 1) * NR + t * L + (r ^ (t & 7)), src);
+                cp_async8_rand(recB + (st & 1) * NR + t * L + (r ^ (t & (L - 1) & 15)), src + 1);
+            }
+        }
     };
 
 #pragma unroll
@@ -422,6 +468,37 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
         };
 
         if (pass > 0) __syncthreads();          // every thread is done with both buffers
+        if constexpr (kIdx) {
+            issue_idx(0);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
+            issue_rec(0);
+            if (1 < n_stage) issue_idx(1);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+#pragma unroll 1
+            for (int st = 0; st < n_stage; ++st) {
+                asm volatile("cp.async.wait_group 0;" ::: "memory");      // records of stage st, indices of stage st + 1
+                __syncthreads();
+                if (st + 1 < n_stage) {
+                    issue_rec(st + 1);
+                    if (st + 2 < n_stage) issue_idx(st + 2);
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+                const long long left = n - (first + (long long)st * L);
+                const int cnt = left >= L ? L : (left > 0 ? (int)left : 0);
+                const uint4* myA = recA + (st & 1) * NR + tid * L;
+                const uint2* myB = recB + (st & 1) * NR + tid * L;
+                const int swB = tid & (L - 1) & 15;
+#pragma unroll 1
+                for (int i = 0; i < cnt; ++i) {
+                    const uint4 a = myA[i ^ sw];
+                    const uint2 c = myB[i ^ swB];
+                    one(a.x, a.y, __uint_as_float(a.z), __uint_as_float(a.w), __uint_as_float(c.x), __uint_as_float(c.y));
+                }
+                __syncthreads();                    // buffer st & 1 is free for stage st + 2
+            }
+        } else {
         issue(0);
 #pragma unroll 1
         for (int st = 0; st < n_stage; ++st) {
@@ -449,19 +526,24 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             }
             __syncthreads();                    // buffer st & 1 is free for stage st + 2
         }
+        }
         if (cij != 0xFFFFFFFFu) flush();
     }
 }
 
-template <int S, int RB, int KIND>
+template <int S, int RB, int KIND, bool kIdx>
 int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
-    constexpr int L = 16;                                   // records per thread and stage
+    // records per thread and stage; 8 in indirect mode: 57 KB of staging, so that two CTAs stay resident (16: 114 KB,
+    // one CTA per SM, measured 48.5 against 40.2 ms on hotspot; a third record buffer -- two stages in flight --
+    // 39.0 against 37.7 ms on hotspot, 12.6 against 13.9 ms on 500M: not kept)
+    constexpr int L = kIdx ? 8 : 16;
     constexpr int NBUF = 2;                                 // double-buffered stages (1 was measured: no gain)
-    constexpr int smem = NBUF * 3 * kRunThreads * (L / 2) * 16;   // NBUF buffers of three streams, 48 KB each
+    // direct: NBUF buffers of three 8-byte streams; indirect: two buffers of 16 + 8 record bytes and 4 index bytes
+    constexpr int smem = kIdx ? 2 * kRunThreads * L * (16 + 8 + 4) : NBUF * 3 * kRunThreads * (L / 2) * 16;
     static bool attr_done[RICK_MAX_DEVICES] = {};      // the opt-in is per device
     const int dv = p->device & (RICK_MAX_DEVICES - 1);
     if (!attr_done[dv]) {
-        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_grid_rec<S, RB, L, NBUF, KIND, kIdx>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return RICK_ECUDA;
         attr_done[dv] = true;
     }
@@ -471,10 +553,10 @@ int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
         tc.Kf[t] = (float)tc.K[t];
     }
     // records per thread: long enough that end-of-range flushes are rare next to run ends (dense inputs
-    // put thousands of visibilities on one cell), short enough for >= ~12 CTAs per SM slot
+    // put thousands of visibilities on one cell), short enough for >= ~12 CTAs per SM slot; at most 256
     const long long want = p->M / ((long long)kRunThreads * p->sm_count * 2 * 12);
     int n_stage = (int)(want / L);
-    n_stage = n_stage < 2 ? 2 : (n_stage > 16 ? 16 : n_stage);
+    n_stage = n_stage < 2 ? 2 : (n_stage > 256 / L ? 256 / L : n_stage);
     const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
     KbPoly kp;
@@ -483,8 +565,8 @@ int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
         memcpy(kp.c, p->kb_poly, sizeof(kp.c));
         kp.ok = 1;
     }
-    k_grid_rec<S, RB, L, NBUF, KIND><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
-                                                           (float2*)grid, n_stage, kp);
+    k_grid_rec<S, RB, L, NBUF, KIND, kIdx><<<blocks, kRunThreads, smem, st>>>(p->g, tc, p->n_kept_dev, p->grec_a, p->grec_b, p->grec_c,
+                                                                 p->gidx, p->grec, (float2*)grid, n_stage, kp);
     return RICK_OK;
 }
 
@@ -508,8 +590,11 @@ void launch_runs_k(rick_plan* p, void* grid, cudaStream_t st) {
 
 template <int S, int RB>
 int launch_rec(rick_plan* p, void* grid, cudaStream_t st) {
-    return p->g.kernel == RICK_KERNEL_KB ? launch_rec_k<S, RB, RICK_KERNEL_KB>(p, grid, st)
-                                         : launch_rec_k<S, RB, RICK_KERNEL_GAUSS>(p, grid, st);
+    if (p->indirect)
+        return p->g.kernel == RICK_KERNEL_KB ? launch_rec_k<S, RB, RICK_KERNEL_KB, true>(p, grid, st)
+                                             : launch_rec_k<S, RB, RICK_KERNEL_GAUSS, true>(p, grid, st);
+    return p->g.kernel == RICK_KERNEL_KB ? launch_rec_k<S, RB, RICK_KERNEL_KB, false>(p, grid, st)
+                                         : launch_rec_k<S, RB, RICK_KERNEL_GAUSS, false>(p, grid, st);
 }
 template <typename real, int S, int RB>
 void launch_runs(rick_plan* p, void* grid, cudaStream_t st) {

@@ -421,7 +421,11 @@ int rick_bin(rick_plan* p, long long M, const float* u, const float* v, const fl
              unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out, void* workspace,
              size_t workspace_bytes, long long* n_kept_dev, void* stream) {
     if (!p || M < 0 || M >= 4294967295ll || !n_kept_dev) return RICK_EINVAL;
-    if (M > 0 && (!u || !v || !w || !vis || !weight || !u_s || !v_s || !w_s || !vis_s || !weight_s)) return RICK_EINVAL;
+    if (M > 0 && (!u || !v || !w || !vis || !weight)) return RICK_EINVAL;
+    // sorted SoA outputs: all five, or none (indirect mode: fp32 mesh only -- the fp64 gridder reads them)
+    const int n_sorted = (u_s != NULL) + (v_s != NULL) + (w_s != NULL) + (vis_s != NULL) + (weight_s != NULL);
+    if (n_sorted != 0 && n_sorted != 5) return RICK_EINVAL;
+    if (n_sorted == 0 && p->dtype == RICK_C128) return RICK_EINVAL;
     if (!workspace || ((uintptr_t)workspace & 255)) return RICK_EINVAL;
     if (workspace_bytes < rick_bin_workspace_bytes(p, M)) return RICK_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;

@@ -84,6 +84,12 @@ struct rick_plan {
     //   a = (i0 | j0 << 16, k), b = (i0 - x, j0 - y) in fp32, c = +-weight * (re, im)
     const uint2* grec_a;
     const float2 *grec_b, *grec_c;
+    // indirect mode (rick_bin without sorted SoA outputs, fp32 mesh): sorted input indices and sort keys (kept
+    // visibilities first) and the staging records in INPUT order, each holding the gridder record
+    // ((i0 | j0 << 16, k, i0 - x, j0 - y), (+-weight re, +-weight im, -, -)); the gridder fetches them by index
+    bool indirect;
+    const uint32_t *gidx, *gkey;
+    const float4* grec;
     // stage timing
     cudaEvent_t ev_start[RICK_T_COUNT], ev_stop[RICK_T_COUNT];
     // rick_image_from_host_chunked: copy stream and the events that hand the two staging halves back and forth

@@ -11,9 +11,26 @@
 
 namespace {
 
+// (j0 << 16 | ., k) of the sorted kept visibility i: from the gridder records, or decoded from the sorted sort keys
+// (indirect mode: sort key = tile key << cb | cell bits, rick_internal.cuh)
+struct RowsFromRecords {
+    const uint2* ga;
+    __device__ __forceinline__ uint2 operator()(const RickGeom&, long long i) const { return __ldg(ga + i); }
+};
+struct RowsFromKeys {
+    const uint32_t* key;
+    __device__ __forceinline__ uint2 operator()(const RickGeom& g, long long i) const {
+        const uint32_t sk = __ldg(key + i);
+        const uint32_t tile = sk >> g.cell_bits, cell = (sk & ((1u << g.cell_bits) - 1u)) << (10 - g.cell_bits);
+        const uint32_t T = (uint32_t)g.T, ty = (tile / T) % T, k = tile / (T * T);
+        return make_uint2((ty * 32u + (cell >> 5)) << 16, k);
+    }
+};
+
 // one thread per sorted kept visibility: the first of every (plane, row j0) group sets the 2h+1 bits
+template <typename Src>
 __global__ void __launch_bounds__(256) k_rows_mark(RickGeom g, const long long* __restrict__ n_kept,
-                                                   const uint2* __restrict__ ga, uint32_t* __restrict__ occ) {
+                                                   Src ga, uint32_t* __restrict__ occ) {
     const long long n = *n_kept;
     const long long stride = (long long)gridDim.x * blockDim.x;
     // four records (and their predecessors) per trip, all loads first: one dependent DRAM wait per four
@@ -26,8 +43,8 @@ __global__ void __launch_bounds__(256) k_rows_mark(RickGeom g, const long long* 
             const long long i = i0 + x * stride;
             a[x] = b[x] = make_uint2(0xffffffffu, 0xffffffffu);          // no record: never a group start's equal
             if (i < n) {
-                a[x] = __ldg(ga + i);
-                if (i > 0) b[x] = __ldg(ga + i - 1);
+                a[x] = ga(g, i);
+                if (i > 0) b[x] = ga(g, i - 1);
             }
         }
 #pragma unroll
@@ -94,7 +111,10 @@ int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
     if (M == 0) return RICK_OK;
     const long long want = (M + 255) / 256;
     const long long cap = (long long)p->sm_count * 16;
-    k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, p->grec_a, p->occ_cur_dev);
+    if (p->indirect)
+        k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromKeys{p->gkey}, p->occ_cur_dev);
+    else
+        k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromRecords{p->grec_a}, p->occ_cur_dev);
     RICK_LAUNCH_CHECK();
     p->launches++;
     return RICK_OK;

@@ -36,12 +36,14 @@ def test_full_plan(name):
     pa = W.plan_args(cfg, vis)
     im = B.Imager(dtype=cfg.dtype, M_max=vis.M, fused=2, **pa)
     assert im.fused == 2
-    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
+    indirect = not im.sorted_outputs          # fp32 mesh: rick_bin gathers nothing, the gridder fetches by index
+    perm = torch.empty(vis.M, dtype=torch.int32, device="cuda") if indirect else None
+    im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight, perm_out=perm)   # in indirect mode perm_out is a copy, not another path
     torch.cuda.synchronize()
     n_kept = int(im.n_kept.item())
     s = im.sorted
-    # checksum: the sorted payload is a permutation of the kept input (sum of bit patterns, exact in int64)
-    kept_sum = int(s["u"][:n_kept].view(torch.int32).to(torch.int64).sum().item())
+    if not indirect:    # checksum: the sorted payload is a permutation of the kept input (sum of bit patterns, exact in int64)
+        kept_sum = int(s["u"][:n_kept].view(torch.int32).to(torch.int64).sum().item())
     im.grid_(True)
     im.fft()
     im.wcorrect(True)
@@ -56,15 +58,26 @@ def test_full_plan(name):
     okey, oi0, oj0, ok, on = O.keys(oplan, *hv)
     assert n_kept == on
     kept = okey < oplan.n_bins
-    assert kept_sum == int(hv[0][kept].view(np.int32).astype(np.int64).sum())
-    # the sorted payload, located again by the oracle, is non-decreasing in the D4' order
-    su, sv, sw = (s[k][:n_kept].cpu().numpy() for k in ("u", "v", "w"))
-    one = np.ones(n_kept, np.complex64)
-    skey, si0, sj0, _, sn = O.keys(oplan, su, sv, sw, one, np.ones(n_kept, np.float32))
-    assert sn == n_kept
-    ssk = (skey.astype(np.int64) * 32 + (sj0 & 31)) * 32 + (si0 & 31)      # D4' order: (plane, tile, row, column)
-    assert np.all(np.diff(ssk) >= 0)
-    del su, sv, sw, one, skey, si0, sj0, ssk, okey, oi0, oj0, ok, kept
+    if indirect:
+        # the sorted index: a permutation of the input, kept visibilities first, non-decreasing in the D4' order
+        pm = perm.cpu().numpy().view(np.uint32).astype(np.int64)
+        del perm
+        assert np.array_equal(np.sort(pm), np.arange(pm.size))
+        assert kept[pm[:n_kept]].all() and not kept[pm[n_kept:]].any()
+        ssk = ((okey.astype(np.int64) * 32 + (oj0 & 31)) * 32 + (oi0 & 31))[pm[:n_kept]]
+        assert np.all(np.diff(ssk) >= 0)
+        del pm, ssk
+    else:
+        assert kept_sum == int(hv[0][kept].view(np.int32).astype(np.int64).sum())
+        # the sorted payload, located again by the oracle, is non-decreasing in the D4' order
+        su, sv, sw = (s[k][:n_kept].cpu().numpy() for k in ("u", "v", "w"))
+        one = np.ones(n_kept, np.complex64)
+        skey, si0, sj0, _, sn = O.keys(oplan, su, sv, sw, one, np.ones(n_kept, np.float32))
+        assert sn == n_kept
+        ssk = (skey.astype(np.int64) * 32 + (sj0 & 31)) * 32 + (si0 & 31)      # D4' order: (plane, tile, row, column)
+        assert np.all(np.diff(ssk) >= 0)
+        del su, sv, sw, one, skey, si0, sj0, ssk
+    del okey, oi0, oj0, ok, kept
     im.close()
     del im, s
     torch.cuda.empty_cache()

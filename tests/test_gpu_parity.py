@@ -102,8 +102,29 @@ BIN_CASES = [
 @pytest.mark.parametrize("name,M,plan,dtype", BIN_CASES)
 def test_bin_bit_exact(name, M, plan, dtype):
     cfg, vis, pa = make(name, M, dtype=dtype, **plan)
-    im = B.Imager(dtype=dtype, M_max=M, alloc_mesh=False, **pa)
+    im = B.Imager(dtype=dtype, M_max=M, alloc_mesh=False, sorted_outputs=True, **pa)
     check_bin(im, vis, pa)
+    im.close()
+
+
+@pytest.mark.parametrize("name,M,plan,dtype", [c for c in BIN_CASES if c[3] == "c64"])
+@pytest.mark.parametrize("fused", [0, 2])
+def test_bin_bit_exact_indirect(name, M, plan, dtype, fused):
+    """rick_bin as bench.py and Imager.run call it on the fp32 mesh: no sorted SoA outputs, so nothing is gathered
+    and the gridder fetches its records through the sorted index (indirect mode).  perm_out is a copy of that
+    index: it must be the oracle's stable D4' permutation, bit for bit; keys, n_kept and bin_start as well."""
+    cfg, vis, pa = make(name, M, dtype=dtype, **plan)
+    im = B.Imager(dtype=dtype, M_max=M, fused=fused, alloc_mesh=False, **pa)
+    assert not im.sorted_outputs
+    u, v, w, vv, wt = vis.numpy()
+    plan_o = O.Plan(**pa)
+    key, perm, bs, n_kept = run_bin(im, vis)
+    okey, oi0, oj0, ok, on = O.keys(plan_o, u, v, w, vv, wt)
+    assert np.array_equal(key, okey) and n_kept == on
+    _, _, cell_bits = B.rick_plan_sort_layout(im.plan)
+    assert np.array_equal(perm, O.sort_cells(oi0, oj0, ok, col_drop=10 - cell_bits))
+    _, obs = O.counting_sort(okey, plan_o.n_bins)
+    assert np.array_equal(bs, obs)
     im.close()
 
 
@@ -113,7 +134,7 @@ def test_bin_bit_exact_fused_gather(name, M, plan, dtype, fused):
     """The variant of rick_bin the timed path runs (gather fused into the last sort pass; fusion mode 2 adds
     the row marking)."""
     cfg, vis, pa = make(name, M, dtype=dtype, **plan)
-    im = B.Imager(dtype=dtype, M_max=M, fused=fused, alloc_mesh=False, **pa)
+    im = B.Imager(dtype=dtype, M_max=M, fused=fused, alloc_mesh=False, sorted_outputs=True, **pa)
     n_kept = check_bin_fused_gather(im, vis, pa)
     assert 0 < n_kept <= M
     im.close()
@@ -137,7 +158,7 @@ def test_sort_many_tiles_and_hot_bin():
     t = lambda a: torch.from_numpy(a).cuda()
     vis = W.Visibilities(t(u), t(v), t(w), torch.ones(M, dtype=torch.complex64, device="cuda"),
                          torch.ones(M, dtype=torch.float32, device="cuda"))
-    im = B.Imager(dtype="c64", M_max=M, **pa)
+    im = B.Imager(dtype="c64", M_max=M, sorted_outputs=True, **pa)
     okey, _, n_kept = check_bin(im, vis, pa)
     assert 0 < n_kept < M and len(np.unique(okey)) > 2000
     im.close()
@@ -494,11 +515,12 @@ def test_split_column_transform(name, M, plan, dtype, fused):
 
 
 @pytest.mark.parametrize("S", [3, 5, 7, 9, 11, 13, 15])
-@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("dtype,sorted_outputs", [("c64", False), ("c64", True), ("c128", True)])
 @pytest.mark.parametrize("kernel", ["gauss", "kb"])
-def test_every_support(S, dtype, kernel):
+def test_every_support(S, dtype, sorted_outputs, kernel):
     """Every footprint width rick_plan_create accepts, both mesh types, both kernels (the multi-pass record
-    gridder for S >= 11 and every k_grid_runs instantiation): mesh and image against the oracle.  The input
+    gridder for S >= 11 in its direct and its indirect form -- with and without the sorted outputs of rick_bin --
+    and every k_grid_runs instantiation): mesh and image against the oracle.  The input
     includes visibilities on the last cells D5 keeps (i0 = h and i0 = N-1-h: the window's zero column falls
     off the row there)."""
     N, Nw, M = 256, 4, 60_000
@@ -514,7 +536,7 @@ def test_every_support(S, dtype, kernel):
     beta = 2.34 * S
     oplan = O.Plan(kernel=kernel, beta=beta, **pa)
     hv = vis.numpy()
-    im = B.Imager(dtype=dtype, M_max=M, kernel=kernel, beta=beta, **pa)
+    im = B.Imager(dtype=dtype, M_max=M, kernel=kernel, beta=beta, sorted_outputs=sorted_outputs, **pa)
     im.bin(vis.u, vis.v, vis.w, vis.vis, vis.weight)
     im.grid_(True)
     torch.cuda.synchronize()
