@@ -208,6 +208,9 @@ def main():
                     help="gridding kernel: the Gaussian of BASELINE.json (default) or the paper's Kaiser-Bessel (beta = 2.34 S)")
     ap.add_argument("--M", type=int, default=0, help="profiling subset: only the first M visibilities of the workload")
     ap.add_argument("--Nw", type=int, default=0, help="profiling subset: this many w-planes instead of the workload's")
+    ap.add_argument("--sorted-outputs", action="store_true",
+                    help="fp32 mesh: ask rick_bin for the sorted SoA copies (the gather runs in the last sort pass and the "
+                         "gridder streams its records) instead of the default indirect mode")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-chunks", type=int, default=4,
                     help="time slices of rick_image_from_host_chunked in the e2e region (1: one copy, then compute)")
@@ -240,10 +243,12 @@ def main():
     vis = W.generate(cfg, device=dev)
     pa = W.plan_args(cfg, vis)
     M = vis.M
-    im = B.Imager(dtype=cfg.dtype, M_max=M, fused=0 if args.no_fusion else args.fusion, kernel=args.kernel, beta=2.34 * cfg.support, **pa)
+    fma_tflops, add_tinst, fma2_tflops = B.rick_measure_fp32_rate()
+    rand_grec = B.rick_measure_random_read_rate()        # before the big buffers exist: it borrows 2 GB
+    im = B.Imager(dtype=cfg.dtype, M_max=M, fused=0 if args.no_fusion else args.fusion, kernel=args.kernel, beta=2.34 * cfg.support,
+                  sorted_outputs=True if (args.sorted_outputs or cfg.dtype == "c128") else None, **pa)
     cell = 16 if cfg.dtype == "c128" else 8
     mesh_bytes = cfg.Nw * cfg.N * cfg.N * cell
-    fma_tflops, add_tinst, fma2_tflops = B.rick_measure_fp32_rate()
 
     def step():
         im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight)
@@ -302,7 +307,7 @@ def main():
         fft_rows_b = 2 * live_bytes if own_rows else 2 * mesh_bytes      # else batched library transforms of every row
         col_a_b = live_bytes + mesh_bytes    # sweep A reads the defined rows, writes every row
         fft_b, wc_b = fft_rows_b + col_a_b, mesh_bytes + cfg.N * cfg.N * 8
-    indirect = cfg.dtype == "c64"       # fp32 mesh: rick_bin gathers nothing; the gridder fetches 32-B records by index
+    indirect = not im.sorted_outputs    # fp32 mesh: rick_bin gathers nothing; the gridder fetches 32-B records by index
     alg = {   # algorithmic bytes per stage
         "keygen": (24 + 4 + 32) * M,                 # SoA in, sort key + 32-B staging record out
         # sort: first pass 4 r + 8 w, middle passes 8 r + 8 w, last pass 8 r and, fused into it, the gather
@@ -365,6 +370,15 @@ def main():
             alu["k_col_a_tflops"] = 5.0 * math.log2(cfg.N // n2) * n_el / (stage_ms["fft_col_a"] * 1e-3) / 1e12
             alu["k_col_b_tflops"] = 5.0 * math.log2(n2) * n_el / (stage_ms["wcorrect"] * 1e-3) / 1e12
     roofline["alu_view"] = alu
+    # the gather (in the last sort pass, or, in indirect mode, inside the gridder) is bound by the GPU's random-access
+    # rate, measured in this run (rick_measure_random_read_rate: random 32-byte records of a 2 GB array)
+    roofline["random_access_view"] = {
+        "measured_grecords_per_s": rand_grec,
+        "gathered_records": n_kept,
+        "floor_ms": n_kept / (rand_grec * 1e9) * 1e3 if rand_grec > 0 else None,
+        "where": "k_grid_rec (indirect mode)" if indirect else "last k_onesweep pass (fused gather)",
+        "grid_stage_grecords_per_s": n_kept / (stage_ms["grid"] * 1e-3) / 1e9 if indirect else None,
+        "frac": (n_kept / (stage_ms["grid"] * 1e-3) / 1e9 / rand_grec) if (indirect and rand_grec > 0) else None}
 
     # end to end through rick_image_from_host(_chunked): pinned host inputs -> host image, copies inside the region
     host = [torch.empty(x.shape, dtype=x.dtype, pin_memory=args.e2e_steps > 0) for x in (vis.u, vis.v, vis.w, vis.vis, vis.weight)]

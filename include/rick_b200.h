@@ -217,6 +217,11 @@ long long rick_launch_count(const rick_plan* plan);
  * bench.py reports issue-bound kernels against these measured numbers. */
 int rick_measure_fp32_rate(double* fma_tflops, double* add_tinst, double* fma2_tflops, void* stream);
 
+/* Measurement helper (host-synchronous; allocates 2 GB of device memory and frees it): how many random 32-byte
+ * records per second (1e9 / s) this GPU reads from a 2 GB array at full occupancy -- the rate that bounds a
+ * gather (the gridder's record fetch in indirect mode). */
+int rick_measure_random_read_rate(double* grecords_per_s, void* stream);
+
 const char* rick_strerror(int status);
 
 #ifdef __cplusplus

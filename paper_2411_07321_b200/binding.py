@@ -24,7 +24,7 @@ EXPORTS = (
     "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_image_from_host_chunked", "rick_get_timings", "rick_launch_count", "rick_strerror",
-    "rick_measure_fp32_rate",
+    "rick_measure_fp32_rate", "rick_measure_random_read_rate",
 )
 
 
@@ -77,6 +77,7 @@ def lib():
         L.rick_launch_count.argtypes = [vp]
         L.rick_launch_count.restype = ll
         L.rick_measure_fp32_rate.argtypes = [C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), vp]
+        L.rick_measure_random_read_rate.argtypes = [C.POINTER(dbl), vp]
         L.rick_strerror.argtypes = [i]
         L.rick_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -225,6 +226,13 @@ def rick_measure_fp32_rate():
     a, b, c = C.c_double(), C.c_double(), C.c_double()
     _check(lib().rick_measure_fp32_rate(C.byref(a), C.byref(b), C.byref(c), _stream()), "rick_measure_fp32_rate")
     return float(a.value), float(b.value), float(c.value)
+
+
+def rick_measure_random_read_rate() -> float:
+    """-> 1e9 random 32-byte records read per second, measured on the current device (measurement helper)."""
+    a = C.c_double()
+    _check(lib().rick_measure_random_read_rate(C.byref(a), _stream()), "rick_measure_random_read_rate")
+    return float(a.value)
 
 
 # ---- buffer ownership helper (allocation + marshalling; no arithmetic) --------------------------

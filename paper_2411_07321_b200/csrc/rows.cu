@@ -19,10 +19,19 @@ struct RowsFromRecords {
 };
 struct RowsFromKeys {
     const uint32_t* key;
+    int log2T;           // >= 0: T = N / 32 is a power of two (shifts instead of two integer divisions per key)
     __device__ __forceinline__ uint2 operator()(const RickGeom& g, long long i) const {
         const uint32_t sk = __ldg(key + i);
         const uint32_t tile = sk >> g.cell_bits, cell = (sk & ((1u << g.cell_bits) - 1u)) << (10 - g.cell_bits);
-        const uint32_t T = (uint32_t)g.T, ty = (tile / T) % T, k = tile / (T * T);
+        uint32_t ty, k;
+        if (log2T >= 0) {
+            ty = (tile >> log2T) & ((1u << log2T) - 1u);
+            k = tile >> (2 * log2T);
+        } else {
+            const uint32_t T = (uint32_t)g.T;
+            ty = (tile / T) % T;
+            k = tile / (T * T);
+        }
         return make_uint2((ty * 32u + (cell >> 5)) << 16, k);
     }
 };
@@ -111,8 +120,11 @@ int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
     if (M == 0) return RICK_OK;
     const long long want = (M + 255) / 256;
     const long long cap = (long long)p->sm_count * 16;
-    if (p->indirect)
-        k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromKeys{p->gkey}, p->occ_cur_dev);
+    if (p->indirect) {
+        int log2T = -1;
+        for (int b = 0; b < 16; ++b) if ((1 << b) == p->g.T) log2T = b;
+        k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromKeys{p->gkey, log2T}, p->occ_cur_dev);
+    }
     else
         k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromRecords{p->grec_a}, p->occ_cur_dev);
     RICK_LAUNCH_CHECK();
