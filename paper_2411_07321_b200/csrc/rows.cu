@@ -20,8 +20,8 @@ struct RowsFromRecords {
 struct RowsFromKeys {
     const uint32_t* key;
     int log2T;           // >= 0: T = N / 32 is a power of two (shifts instead of two integer divisions per key)
-    __device__ __forceinline__ uint2 operator()(const RickGeom& g, long long i) const {
-        const uint32_t sk = __ldg(key + i);
+    __device__ __forceinline__ uint2 operator()(const RickGeom& g, long long i) const { return decode(g, __ldg(key + i)); }
+    __device__ __forceinline__ uint2 decode(const RickGeom& g, uint32_t sk) const {
         const uint32_t tile = sk >> g.cell_bits, cell = (sk & ((1u << g.cell_bits) - 1u)) << (10 - g.cell_bits);
         uint32_t ty, k;
         if (log2T >= 0) {
@@ -35,6 +35,20 @@ struct RowsFromKeys {
         return make_uint2((ty * 32u + (cell >> 5)) << 16, k);
     }
 };
+
+// rows j0-h .. j0+h of plane k as one or two word masks; bits only ever get set, so a plain (L2) read that
+// already shows them saves the atomic: the many tiles of a mesh row would otherwise all hit one word
+__device__ __forceinline__ void mark_rows(const RickGeom& g, uint32_t j0, uint32_t k, uint32_t* __restrict__ occ) {
+    const uint32_t lo = k * (uint32_t)g.N + (j0 - (uint32_t)g.h), hi = lo + 2u * (uint32_t)g.h;
+    const uint32_t w0 = lo >> 5, w1 = hi >> 5;
+    const uint32_t span = (2u * (uint32_t)g.h + 1u);
+    const uint32_t m0 = (span >= 32u ? 0xffffffffu : ((1u << span) - 1u)) << (lo & 31);
+    if ((__ldcg(occ + w0) & m0) != m0) atomicOr(occ + w0, m0);
+    if (w1 != w0) {
+        const uint32_t m1 = (1u << ((hi & 31) + 1u)) - 1u;
+        if ((__ldcg(occ + w1) & m1) != m1) atomicOr(occ + w1, m1);
+    }
+}
 
 // one thread per sorted kept visibility: the first of every (plane, row j0) group sets the 2h+1 bits
 template <typename Src>
@@ -61,17 +75,35 @@ __global__ void __launch_bounds__(256) k_rows_mark(RickGeom g, const long long* 
             if (i0 + x * stride >= n) break;
             const uint32_t j0 = a[x].x >> 16, k = a[x].y;
             if ((b[x].x >> 16) == j0 && b[x].y == k) continue;
-            // rows j0-h .. j0+h as one or two word masks; bits only ever get set, so a plain (L2) read that
-            // already shows them saves the atomic: the many tiles of a mesh row would otherwise all hit one word
-            const uint32_t lo = k * (uint32_t)g.N + (j0 - (uint32_t)g.h), hi = lo + 2u * (uint32_t)g.h;
-            const uint32_t w0 = lo >> 5, w1 = hi >> 5;
-            const uint32_t span = (2u * (uint32_t)g.h + 1u);
-            const uint32_t m0 = (span >= 32u ? 0xffffffffu : ((1u << span) - 1u)) << (lo & 31);
-            if ((__ldcg(occ + w0) & m0) != m0) atomicOr(occ + w0, m0);
-            if (w1 != w0) {
-                const uint32_t m1 = (1u << ((hi & 31) + 1u)) - 1u;
-                if ((__ldcg(occ + w1) & m1) != m1) atomicOr(occ + w1, m1);
-            }
+            mark_rows(g, j0, k, occ);
+        }
+    }
+}
+
+// The same from the sorted sort keys (indirect mode), eight consecutive keys per thread and trip with two 16-byte
+// loads: a key with its column bits shifted out names its (plane, tile, row); only the first key of every such
+// group decodes and marks.  (One key per thread through the generic kernel waited on its two dependent loads:
+// 2.8 ms on hotspot.)
+__global__ void __launch_bounds__(256) k_rows_mark_keys(RickGeom g, const long long* __restrict__ n_kept,
+                                                        const uint32_t* __restrict__ key, int log2T,
+                                                        uint32_t* __restrict__ occ) {
+    const long long n = *n_kept;
+    const int col_bits = g.cell_bits - 5;                 // cell_bits >= 5: the row-in-tile bits are always kept
+    const RowsFromKeys dec{key, log2T};
+    const long long stride = (long long)gridDim.x * blockDim.x * 8;
+    for (long long base = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 8; base < n; base += stride) {
+        // the key array is padded to whole multiples of 4096 entries: the two loads stay inside it
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(key + base));
+        const uint4 b = __ldg(reinterpret_cast<const uint4*>(key + base + 4));
+        const uint32_t prev = base > 0 ? __ldg(key + base - 1) : 0u;
+        const uint32_t k8[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            if (base + x >= n) break;
+            const uint32_t before = x ? k8[x - 1] : prev;
+            if ((base + x > 0) && (before >> col_bits) == (k8[x] >> col_bits)) continue;
+            const uint2 r = dec.decode(g, k8[x]);
+            mark_rows(g, r.x >> 16, r.y, occ);
         }
     }
 }
@@ -123,7 +155,8 @@ int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
     if (p->indirect) {
         int log2T = -1;
         for (int b = 0; b < 16; ++b) if ((1 << b) == p->g.T) log2T = b;
-        k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromKeys{p->gkey, log2T}, p->occ_cur_dev);
+        const long long want8 = (M / 8 + 255) / 256 + 1;
+        k_rows_mark_keys<<<(int)(want8 > cap ? cap : want8), 256, 0, st>>>(p->g, p->n_kept_dev, p->gkey, log2T, p->occ_cur_dev);
     }
     else
         k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromRecords{p->grec_a}, p->occ_cur_dev);
