@@ -25,9 +25,9 @@ template <typename C2, int N1, int N2> struct RowBig {
     static constexpr int PB = N1 + 1;                                  // pitch of the transposed layout
     static constexpr size_t elems = (size_t)N2 * PB;                   // >= N
     static constexpr size_t smem = sizeof(C2) * (elems + N1 + N2);
-    // resident CTAs per SM the register allocation leaves room for: by shared memory, at >= 128 registers per thread
+    // resident CTAs per SM the register allocation leaves room for: by shared memory, at 128 (fp32) / 255 (fp64) registers per thread
     static constexpr int kBySmem = (int)((227 * 1024) / (smem + 1024));
-    static constexpr int kByRegs = 65536 / (T * 128);
+    static constexpr int kByRegs = 65536 / (T * (sizeof(C2) == 16 ? 255 : 128));      // 32 complex values per thread: 64 / 128 registers
     static constexpr int kMinBlocks = kBySmem < kByRegs ? (kBySmem < 1 ? 1 : kBySmem) : (kByRegs < 1 ? 1 : kByRegs);
 };
 

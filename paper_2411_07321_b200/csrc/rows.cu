@@ -20,7 +20,6 @@ struct RowsFromRecords {
 struct RowsFromKeys {
     const uint32_t* key;
     int log2T;           // >= 0: T = N / 32 is a power of two (shifts instead of two integer divisions per key)
-    __device__ __forceinline__ uint2 operator()(const RickGeom& g, long long i) const { return decode(g, __ldg(key + i)); }
     __device__ __forceinline__ uint2 decode(const RickGeom& g, uint32_t sk) const {
         const uint32_t tile = sk >> g.cell_bits, cell = (sk & ((1u << g.cell_bits) - 1u)) << (10 - g.cell_bits);
         uint32_t ty, k;
