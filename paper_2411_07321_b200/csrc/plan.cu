@@ -376,8 +376,10 @@ int rick_plan_workspace_bytes(const rick_plan* p, long long M, size_t* bin_bytes
     if (bin_bytes) *bin_bytes = rick_bin_workspace_bytes(p, M);
     if (fft_bytes) {
         if (!p->fft_ready) return RICK_ESTATE;
-        // fused: only the batched row transforms go through cuFFT
-        *fft_bytes = p->fused ? p->fft_rows_work_bytes : p->fft_work_bytes;
+        // fused: only the batched row transforms go through cuFFT -- and in mode 2 not even those where the library
+        // has a row kernel of its own (k_rowfft, k_row_big)
+        const bool own_rows = p->fused == 2 && (!p->split || rick_rowbig_supported(p));
+        *fft_bytes = p->fused ? (own_rows ? 0 : p->fft_rows_work_bytes) : p->fft_work_bytes;
     }
     return RICK_OK;
 }
