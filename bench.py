@@ -212,7 +212,7 @@ def main():
                     help="fp32 mesh: ask rick_bin for the sorted SoA copies (the gather runs in the last sort pass and the "
                          "gridder streams its records) instead of the default indirect mode")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--e2e-chunks", type=int, default=4,
+    ap.add_argument("--e2e-chunks", type=int, default=8,
                     help="time slices of rick_image_from_host_chunked in the e2e region (1: one copy, then compute)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup

@@ -193,9 +193,9 @@ int rick_image_from_host(rick_plan* plan, long long M, const float* u_host, cons
  * rick_wcorrect_accumulate and the image copy.  The staging arrays of `dev` (capacity M) are used as two
  * halves, so a slice holds at most M/2 visibilities (rounded to a multiple of 1024); n_chunks < 2 or
  * M < 2048 falls back to rick_image_from_host.  The image equals the single-slice one up to the order of
- * the floating-point additions on the mesh.  With the fused column kernel (rick_plan_set_fusion) the image
- * is computed in up to four parts of whole columns, each copied to image_host by the second stream while the
- * next part is computed.  Returns after synchronising `stream` and the copies. */
+ * the floating-point additions on the mesh.  With the fused column kernels (rick_plan_set_fusion) the image
+ * is computed in up to four stripes of whole columns, each copied to image_host by the second stream while the
+ * next stripe is computed.  Returns after synchronising `stream` and the copies. */
 int rick_image_from_host_chunked(rick_plan* plan, long long M, const float* u_host, const float* v_host,
                                  const float* w_host, const void* vis_host, const float* weight_host,
                                  const rick_device_buffers* dev, int n_chunks, double* image_host,

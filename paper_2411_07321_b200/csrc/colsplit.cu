@@ -208,7 +208,7 @@ template <typename C2, int L> struct ColB {
 template <typename C2, int N1, int N2>
 __global__ void __launch_bounds__(ColB<C2, N2>::T, ColB<C2, N2>::kMinBlocks)
 k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, const double* __restrict__ inv_t,
-        double* __restrict__ image, int accumulate) {
+        double* __restrict__ image, int accumulate, int col_first) {
     typedef typename RickRealOf<C2>::type real;
     constexpr int L = N2, N = N1 * N2;
     typedef ColB<C2, L> P;
@@ -222,7 +222,7 @@ k_col_b(RickGeom g, const C2* __restrict__ planes, const C2* __restrict__ tw_g, 
     const int tid = threadIdx.x, c = tid % C, gq = tid / C;
     const int b = blockIdx.y;                                       // block of L consecutive mesh rows
     const int q1 = slot_freq<N1>(b);                                // the frequency sweep A left there
-    const int col0 = blockIdx.x * C, p = col0 + c;
+    const int col0 = col_first + blockIdx.x * C, p = col0 + c;     // col_first: first column of this launch's part of the image
     const C2* src0 = planes + (size_t)b * L * N + col0;             // row 0 of the tile in plane 0
 
     if (tid == 0) {
@@ -324,7 +324,7 @@ int launch_a(rick_plan* p, void* grid, cudaStream_t st) {
 }
 
 template <typename C2, int N1, int N2>
-int launch_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st) {
+int launch_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st, int col_lo, int col_hi) {
     typedef ColB<C2, N2> P;
     constexpr int N = N1 * N2;
     static bool attr_done[RICK_MAX_DEVICES] = {};
@@ -334,9 +334,11 @@ int launch_b(rick_plan* p, const void* grid, double* image, int accumulate, cuda
             return RICK_ECUDA;
         done = true;
     }
-    const dim3 blocks((unsigned)(N / P::C), (unsigned)N1);
+    if (col_hi < 0) col_hi = N;
+    if (col_lo < 0 || col_hi > N || col_lo >= col_hi || (col_lo % P::C) || (col_hi % P::C)) return RICK_EINVAL;
+    const dim3 blocks((unsigned)((col_hi - col_lo) / P::C), (unsigned)N1);
     k_col_b<C2, N1, N2><<<blocks, P::T, P::smem, st>>>(p->g, (const C2*)grid, (const C2*)p->split_tw, p->inv_taper_dev,
-                                                        image, accumulate);
+                                                        image, accumulate, col_lo);
     return RICK_OK;
 }
 
@@ -360,8 +362,8 @@ int sweep_a(rick_plan* p, void* grid, cudaStream_t st) {
 #undef RICK_CALL_A
 }
 template <typename C2>
-int sweep_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st) {
-#define RICK_CALL_B(n1, n2) launch_b<C2, n1, n2>(p, grid, image, accumulate, st)
+int sweep_b(rick_plan* p, const void* grid, double* image, int accumulate, cudaStream_t st, int col_lo, int col_hi) {
+#define RICK_CALL_B(n1, n2) launch_b<C2, n1, n2>(p, grid, image, accumulate, st, col_lo, col_hi)
     RICK_SPLIT_DISPATCH(RICK_CALL_B)
 #undef RICK_CALL_B
 }
@@ -413,10 +415,13 @@ int rick_colsplit_a_impl(rick_plan* p, void* grid, cudaStream_t st) {
     return RICK_OK;
 }
 
-// sweep B + phase screen + plane sum + taper (rick_wcorrect_accumulate)
-int rick_colsplit_b_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st) {
+// sweep B + phase screen + plane sum + taper (rick_wcorrect_accumulate) for the image columns [col_lo, col_hi)
+// (multiples of 64; col_hi < 0: all): the chunked host entry copies one part out while the next is computed
+int rick_colsplit_b_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st, int col_lo,
+                         int col_hi) {
     const int acc = zero_first ? 0 : 1;
-    const int rc = p->dtype == RICK_C128 ? sweep_b<double2>(p, grid, image, acc, st) : sweep_b<float2>(p, grid, image, acc, st);
+    const int rc = p->dtype == RICK_C128 ? sweep_b<double2>(p, grid, image, acc, st, col_lo, col_hi)
+                                         : sweep_b<float2>(p, grid, image, acc, st, col_lo, col_hi);
     if (rc != RICK_OK) return rc;
     RICK_LAUNCH_CHECK();
     p->launches++;

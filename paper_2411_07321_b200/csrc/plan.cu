@@ -609,6 +609,24 @@ int rick_image_from_host_chunked(rick_plan* p, long long M, const float* u_h, co
         if ((rc = rick_grid(p, d->grid, i == 0, stream)) != RICK_OK) return rc;
     }
     if ((rc = rick_fft_planes(p, d->grid, d->fft_work, d->fft_work_bytes, stream)) != RICK_OK) return rc;
+    if (p->fused && p->split && p->g.N >= 1024) {
+        // split engine: sweep B over RICK_IMAGE_PARTS column stripes; the copy stream takes a stripe to the host while
+        // the next one is computed
+        const int N = p->g.N, stripe = N / RICK_IMAGE_PARTS;
+        StageTimer tm(p, RICK_T_WCORRECT, st);
+        for (int part = 0; part < RICK_IMAGE_PARTS; ++part) {
+            const int c_lo = part * stripe, c_hi = c_lo + stripe;
+            if ((rc = rick_colsplit_b_impl(p, d->grid, d->image, 1, st, c_lo, c_hi)) != RICK_OK) return rc;
+            RICK_CUDA(cudaEventRecord(p->ev_part[part], st));
+            RICK_CUDA(cudaStreamWaitEvent(cs, p->ev_part[part], 0));
+            RICK_CUDA(cudaMemcpy2DAsync(image_host + c_lo, sizeof(double) * (size_t)N, d->image + c_lo,
+                                        sizeof(double) * (size_t)N, sizeof(double) * (size_t)stripe, (size_t)N,
+                                        cudaMemcpyDeviceToHost, cs));
+        }
+        RICK_CUDA(cudaStreamSynchronize(st));
+        RICK_CUDA(cudaStreamSynchronize(cs));
+        return RICK_OK;
+    }
     if (!p->fused || p->split) {
         if ((rc = rick_wcorrect_accumulate(p, d->grid, d->image, 1, stream)) != RICK_OK) return rc;
         if ((rc = rick_image(p, d->image, image_host, 1, stream)) != RICK_OK) return rc;

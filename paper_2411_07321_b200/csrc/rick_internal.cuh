@@ -196,7 +196,8 @@ int rick_colfft_columns_per_cta();
 bool rick_colsplit_supported(const rick_plan* p);
 int rick_colsplit_init(rick_plan* p);
 int rick_colsplit_a_impl(rick_plan* p, void* grid, cudaStream_t st);
-int rick_colsplit_b_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st);
+int rick_colsplit_b_impl(rick_plan* p, const void* grid, double* image, int zero_first, cudaStream_t st,
+                         int col_lo = 0, int col_hi = -1);
 bool rick_rowbig_supported(const rick_plan* p);
 int rick_rowbig_impl(rick_plan* p, void* grid, cudaStream_t st);         // row transforms of the listed rows, N >= 4096
 int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st);          // rick_bin: occ_cur from the records

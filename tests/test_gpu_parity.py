@@ -328,6 +328,8 @@ def test_chunked_accumulation_and_host_entry():
     (2, 700_001, dict(N=512, Nw=8)),
     (1, 1_000_003, dict(N=2048, Nw=32)),       # the bench plan: the image leaves in four parts
     (2, 1_000_003, dict(N=2048, Nw=32)),
+    (2, 400_003, dict(N=4096, Nw=3)),          # split column transform: sweep B leaves in four column stripes
+    (1, 400_003, dict(N=4096, Nw=3)),
 ])
 def test_image_from_host_chunked_c64(fused, M, plan):
     """rick_image_from_host_chunked on the c64 mesh, plain and with row occupancy (fusion mode 2):
