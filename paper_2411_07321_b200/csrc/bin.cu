@@ -208,10 +208,11 @@ __device__ __forceinline__ void gather_one(const GatherOut& o, size_t src, size_
     o.gc[pos] = make_float2(ws * a.w, ws * b.x);
 }
 
-struct SortSmem {
-    uint32_t warp_cnt[kSortWarps][kRadix];   // per-warp digit counts -> exclusive offsets over warps
-    uint32_t tile_excl[kRadix];              // first slot of each digit in the exchanged tile
-    uint32_t glob[kRadix];                   // global position of slot i of digit d = glob[d] + i
+// sized by the digit width: 74 KB for 8-bit digits (three CTAs per SM), 84 KB for 9-bit digits (two)
+template <int kBits> struct SortSmem {
+    uint32_t warp_cnt[kSortWarps][1 << kBits];   // per-warp digit counts -> exclusive offsets over warps
+    uint32_t tile_excl[1 << kBits];              // first slot of each digit in the exchanged tile
+    uint32_t glob[1 << kBits];                   // global position of slot i of digit d = glob[d] + i
     uint32_t xkey[kSortTile];
     uint32_t xidx[kSortTile];
     uint32_t warp_sum[kSortWarps];
@@ -221,8 +222,12 @@ struct SortSmem {
 // kGather: this is the last pass and nobody asked for the sorted (key, index) arrays: instead of writing them,
 // the tile gathers its visibilities straight to their final positions (the gather's random reads hide
 // under the pass's arithmetic, and 12 bytes per visibility of key/index traffic disappear).
+// Registers: only the keys and their ranks live through the ranking loop (the kernel is latency-bound: resident
+// warps are what it needs -- three CTAs per SM for the plain 8-bit passes, 23.0 -> 21.6 ms for the four passes of
+// hotspot; the gather variant keeps two CTAs of 128 registers, it needs them for the fp64 coordinates); the keys go to their exchange slots before the look-back, and the input indices are
+// loaded only then, in flight during the look-back, and follow into the slots the ranks (now slot numbers) name.
 template <bool kFirst, int kBits, bool kGather>
-__global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __restrict__ key_in,
+__global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2) k_onesweep(const uint32_t* __restrict__ key_in,
                                                                const uint32_t* __restrict__ idx_in,
                                                                uint32_t* __restrict__ key_out,
                                                                uint32_t* __restrict__ idx_out, long long M, int shift,
@@ -231,10 +236,10 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
                                                                uint32_t* __restrict__ ticket, uint32_t epoch,
                                                                GatherOut go) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem& sm = *reinterpret_cast<SortSmem*>(smem_raw);
+    SortSmem<kBits>& sm = *reinterpret_cast<SortSmem<kBits>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < kSortWarps * kRadix; i += kSortThreads) (&sm.warp_cnt[0][0])[i] = 0;
+    for (int i = tid; i < kSortWarps * (1 << kBits); i += kSortThreads) (&sm.warp_cnt[0][0])[i] = 0;
     __syncthreads();
     const uint32_t tile = sm.tile;
     const long long tile_base = (long long)tile * kSortTile;
@@ -243,8 +248,8 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
     constexpr int kDigitsPerThread = (1 << kBits) / kSortThreads;   // 2 (9-bit digits) or 1 (8-bit digits)
     static_assert(kDigitsPerThread >= 1, "digit width too small for the block size");
 
-    uint32_t k[kSortItems], id[kSortItems];
-    uint16_t rank[kSortItems];
+    uint32_t k[kSortItems];
+    uint16_t rank[kSortItems];              // rank in the warp's digit bucket, later the exchange slot (< 8192)
     const unsigned lt = (1u << lane) - 1u;
     const bool full = tile_base + kSortTile <= M;     // every tile but the last: no validity tests
     // rank of an item among the items of its warp with the same digit (stable: lanes in order), by one
@@ -256,7 +261,6 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
             const long long gidx = base + j * 32;
             const bool valid = kFull || gidx < M;
             k[j] = valid ? __ldg(key_in + gidx) : 0u;
-            id[j] = kFirst ? (uint32_t)gidx : (valid ? __ldg(idx_in + gidx) : 0u);
         }
 #pragma unroll
         for (int j = 0; j < kSortItems; ++j) {
@@ -336,6 +340,25 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
         sm.tile_excl[tid * kDigitsPerThread + q] = excl_tile;
         excl_tile += tot[q];
     }
+    __syncthreads();                                  // tile_excl and the warp offsets are complete
+    // the keys take their places in digit order now: the ranks become slot numbers and the key registers are free
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+        const bool valid = full || (base + j * 32) < M;
+        if (valid) {
+            const uint32_t d = (k[j] >> shift) & mask;
+            const uint32_t lp = sm.tile_excl[d] + sm.warp_cnt[warp][d] + rank[j];
+            sm.xkey[lp] = k[j];
+            rank[j] = (uint16_t)lp;
+        }
+    }
+    // the input indices, in flight during the look-back
+    uint32_t id[kSortItems];
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+        const long long gidx = base + j * 32;
+        id[j] = kFirst ? (uint32_t)gidx : ((full || gidx < M) ? __ldg(idx_in + gidx) : 0u);
+    }
     // decoupled look-back: a window of kLookWin predecessors per digit is loaded at once (independent
     // loads in flight), then consumed from the nearest tile backwards up to the first inclusive prefix
     if (tile != 0) {
@@ -386,17 +409,10 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint32_t* __
             sm.glob[d] = digit_base[d] - texcl[q];
         }
     }
-    __syncthreads();
-    // exchange into digit order
+    // the indices follow the keys into digit order
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        const bool valid = full || (base + j * 32) < M;
-        if (valid) {
-            const uint32_t d = (k[j] >> shift) & mask;
-            const uint32_t lp = sm.tile_excl[d] + sm.warp_cnt[warp][d] + rank[j];
-            sm.xkey[lp] = k[j];
-            sm.xidx[lp] = id[j];
-        }
+        if (full || (base + j * 32) < M) sm.xidx[rank[j]] = id[j];
     }
     __syncthreads();
     const long long left = M - tile_base;
@@ -448,16 +464,16 @@ size_t rick_bin_workspace_bytes(const rick_plan* p, long long M) {
 }
 
 int rick_bin_init() {
-    const int bytes = (int)sizeof(SortSmem);
+    const int b8 = (int)sizeof(SortSmem<8>), b9 = (int)sizeof(SortSmem<9>);
     const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
-    if (cudaFuncSetAttribute(k_onesweep<true, 8, false>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 9, false>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 8, false>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 9, false>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 8, true>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 9, true>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 8, true>, a, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 9, true>, a, bytes) != cudaSuccess)
+    if (cudaFuncSetAttribute(k_onesweep<true, 8, false>, a, b8) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, false>, a, b9) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, false>, a, b8) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, false>, a, b9) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 8, true>, a, b8) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, true>, a, b9) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, true>, a, b8) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, true>, a, b9) != cudaSuccess)
         return RICK_ECUDA;
     return RICK_OK;
 }
@@ -524,7 +540,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
                                       : (nine ? k_onesweep<false, 9, true> : k_onesweep<false, 8, true>))
                              : (first ? (nine ? k_onesweep<true, 9, false> : k_onesweep<true, 8, false>)
                                       : (nine ? k_onesweep<false, 9, false> : k_onesweep<false, 8, false>));
-            kern<<<n_tiles, kSortThreads, sizeof(SortSmem), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
+            kern<<<n_tiles, kSortThreads, nine ? sizeof(SortSmem<9>) : sizeof(SortSmem<8>), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
                                                                  ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
                                                                  (uint32_t)(pass + 1), go);
             RICK_LAUNCH_CHECK();
