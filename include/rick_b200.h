@@ -52,7 +52,8 @@ typedef enum {
     RICK_ENOMEM = -2,  /* a caller-provided workspace is too small, or plan allocation failed */
     RICK_ECUDA = -3,   /* a CUDA runtime call or kernel launch failed */
     RICK_ECUFFT = -4,  /* a cuFFT call failed */
-    RICK_ESTATE = -5   /* call order: rick_grid before rick_bin, FFT before rick_plan_set_dtype, ... */
+    RICK_ESTATE = -5,  /* call order: rick_grid before rick_bin, FFT before rick_plan_set_dtype, ... */
+    RICK_ELIMIT = -6   /* rick_bin_static: M exceeds RICK_BIN_STATIC_MAX_M, the capacity of the library's static scratch */
 } rick_status;
 
 typedef enum { RICK_C64 = 0, RICK_C128 = 1 } rick_dtype;
@@ -146,6 +147,29 @@ int rick_bin(rick_plan* plan, long long M, const float* u, const float* v, const
              const void* vis, const float* weight, float* u_s, float* v_s, float* w_s, void* vis_s,
              float* weight_s, unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out,
              void* workspace, size_t workspace_bytes, long long* n_kept_dev, void* stream);
+
+/* rick_bin without a caller workspace, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * serving loops, harnesses that forbid allocation): the same kernels, the same arguments minus `workspace`, the same
+ * outputs [D2-D5]; the scratch (sort keys and indices, staging records, digit histograms, look-back words: about
+ * 64.5 bytes per visibility) lives in ONE file-scope device array of the library, RICK_BIN_STATIC_BYTES (17 MiB),
+ * which every GPU that loads the library holds until the process exits.
+ *   M    0 <= M <= RICK_BIN_STATIC_MAX_M (262144); a larger M is refused with RICK_ELIMIT before anything is enqueued
+ *        (use rick_bin with a workspace of your own for larger inputs)
+ * The call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating library routine): it looks up the
+ * array's device address once per device (cudaGetSymbolAddress, with the plan's device current -- RICK_EINVAL if
+ * another device is current) and hands it to rick_bin's kernels.  Everything else is rick_bin: the plan is bound
+ * to the static scratch until the last rick_grid that uses it.
+ * The array is shared by EVERY plan and every call on that device and keeps the last call's contents; the call
+ * clears the part that must start at zero (histograms, tickets, look-back words) itself, on `stream`.  Two calls
+ * (or one call and a rick_grid bound to an earlier one) that overlap on the GPU -- different streams, or two host
+ * threads -- race on it: order them on one stream or with events.
+ * Errors: those of rick_bin, plus RICK_ELIMIT. */
+#define RICK_BIN_STATIC_MAX_M 262144
+#define RICK_BIN_STATIC_BYTES (17u << 20)
+int rick_bin_static(rick_plan* plan, long long M, const float* u, const float* v, const float* w,
+                    const void* vis, const float* weight, float* u_s, float* v_s, float* w_s, void* vis_s,
+                    float* weight_s, unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out,
+                    long long* n_kept_dev, void* stream);
 
 /* Gridding, Eq. 3 [D6], of the visibilities bound by the last rick_bin into
  * grid[Nw][N][N] (device, dtype of the plan, caller-owned).  zero_first != 0 clears the mesh first;

@@ -24,7 +24,7 @@ EXPORTS = (
     "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_image_from_host_chunked", "rick_get_timings", "rick_launch_count", "rick_strerror",
-    "rick_measure_fp32_rate", "rick_measure_random_read_rate",
+    "rick_measure_fp32_rate", "rick_measure_random_read_rate", "rick_bin_static",
 )
 
 
@@ -67,6 +67,7 @@ def lib():
         L.rick_plan_rows_defined.argtypes = [vp, C.POINTER(ll)]
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
+        L.rick_bin_static.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, vp]
         L.rick_grid.argtypes = [vp, vp, i, vp]
         L.rick_fft_planes.argtypes = [vp, vp, vp, sz, vp]
         L.rick_wcorrect_accumulate.argtypes = [vp, vp, vp, i, vp]
@@ -184,6 +185,32 @@ def rick_bin(plan: int, M: int, u, v, w, vis, weight, u_s, v_s, w_s, vis_s, weig
                           _ptr(w_s), _ptr(vis_s), _ptr(weight_s), _ptr(key_out), _ptr(perm_out),
                           _ptr(bin_start_out), _ptr(workspace), workspace.numel(), _ptr(n_kept), _stream(stream)),
            "rick_bin")
+
+
+RICK_BIN_STATIC_MAX_M = 262144
+
+
+def rick_bin_static(plan: int, M: int, u, v, w, vis, weight, u_s, v_s, w_s, vis_s, weight_s, n_kept,
+                    key_out=None, perm_out=None, bin_start_out=None, stream=None) -> None:
+    """rick_bin with the library's static device scratch instead of a caller workspace: allocates nothing,
+    M <= RICK_BIN_STATIC_MAX_M (RICK_ELIMIT beyond), calls that overlap on the GPU race (rick_b200.h)."""
+    f32, c64 = torch.float32, torch.complex64
+    for t, dt, nm in ((u, f32, "u"), (v, f32, "v"), (w, f32, "w"), (vis, c64, "vis"), (weight, f32, "weight")):
+        _dev(t, dt, min(M, RICK_BIN_STATIC_MAX_M), nm)
+    for t, dt, nm in ((u_s, f32, "u_s"), (v_s, f32, "v_s"), (w_s, f32, "w_s"), (vis_s, c64, "vis_s"),
+                      (weight_s, f32, "weight_s")):
+        if t is not None:
+            _dev(t, dt, min(M, RICK_BIN_STATIC_MAX_M), nm)
+    _dev(n_kept, torch.int64, 1, "n_kept")
+    if key_out is not None:
+        _dev(key_out, torch.int32, min(M, RICK_BIN_STATIC_MAX_M), "key_out")
+    if perm_out is not None:
+        _dev(perm_out, torch.int32, min(M, RICK_BIN_STATIC_MAX_M), "perm_out")
+    if bin_start_out is not None:
+        _dev(bin_start_out, torch.int64, None, "bin_start_out")
+    _check(lib().rick_bin_static(plan, M, _ptr(u), _ptr(v), _ptr(w), _ptr(vis), _ptr(weight), _ptr(u_s), _ptr(v_s),
+                                 _ptr(w_s), _ptr(vis_s), _ptr(weight_s), _ptr(key_out), _ptr(perm_out),
+                                 _ptr(bin_start_out), _ptr(n_kept), _stream(stream)), "rick_bin_static")
 
 
 def rick_grid(plan: int, grid: torch.Tensor, zero_first: bool = True, stream=None) -> None:

@@ -602,3 +602,42 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
     p->bound = true;
     return RICK_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// rick_bin_static (rick_b200.h): rick_bin for callers that cannot allocate.  The workspace rick_bin_impl carves
+// (sort keys and indices, staging records, histograms, tickets, look-back words) is this file-scope device array.
+// Every GPU that loads the library holds it until exit; every plan and call on a device shares it, and it keeps
+// the last call's contents: rick_bin_impl clears the region that must start at zero on the caller's stream, as it
+// does for a caller workspace.  Calls that overlap on the GPU race on it (rick_b200.h).
+// In host code the array's name is a host-side stand-in, not a device address: the address handed to the kernels
+// comes from cudaGetSymbolAddress, looked up once per device with that device current.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char rick_bin_static_scratch[RICK_BIN_STATIC_BYTES];
+
+extern "C" int rick_bin_static(rick_plan* p, long long M, const float* u, const float* v, const float* w,
+                               const void* vis, const float* weight, float* u_s, float* v_s, float* w_s, void* vis_s,
+                               float* weight_s, unsigned* key_out, unsigned* perm_out, unsigned long long* bin_start_out,
+                               long long* n_kept_dev, void* stream) {
+    if (!p || M < 0 || !n_kept_dev) return RICK_EINVAL;
+    if (M > RICK_BIN_STATIC_MAX_M || carve(nullptr, M).total > (size_t)RICK_BIN_STATIC_BYTES) return RICK_ELIMIT;
+    if (M > 0 && (!u || !v || !w || !vis || !weight)) return RICK_EINVAL;
+    const int n_sorted = (u_s != nullptr) + (v_s != nullptr) + (w_s != nullptr) + (vis_s != nullptr) + (weight_s != nullptr);
+    if (n_sorted != 0 && n_sorted != 5) return RICK_EINVAL;
+    if (n_sorted == 0 && p->dtype == RICK_C128) return RICK_EINVAL;
+    int dev = -1;
+    RICK_CUDA(cudaGetDevice(&dev));
+    if (dev != p->device || dev < 0 || dev >= RICK_MAX_DEVICES) return RICK_EINVAL;   // the look-up below needs the plan's device current
+    static void* scratch_of_device[RICK_MAX_DEVICES] = {};
+    void* scratch = scratch_of_device[dev];
+    if (!scratch) {
+        RICK_CUDA(cudaGetSymbolAddress(&scratch, rick_bin_static_scratch));
+        if (!scratch || ((uintptr_t)scratch & 255)) return RICK_ECUDA;
+        scratch_of_device[dev] = scratch;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    rick_stage_begin(p, RICK_T_BIN, st);
+    const int rc = rick_bin_impl(p, M, u, v, w, (const float2*)vis, weight, u_s, v_s, w_s, (float2*)vis_s, weight_s,
+                                 key_out, perm_out, bin_start_out, scratch, n_kept_dev, st);
+    rick_stage_end(p, RICK_T_BIN, st);
+    return rc;
+}

@@ -685,6 +685,7 @@ const char* rick_strerror(int status) {
         case RICK_ECUDA: return "CUDA runtime error";
         case RICK_ECUFFT: return "cuFFT error";
         case RICK_ESTATE: return "call order violated (bind/dtype missing)";
+        case RICK_ELIMIT: return "M exceeds RICK_BIN_STATIC_MAX_M, the capacity of the static scratch (use rick_bin with a workspace)";
         default: return "unknown status";
     }
 }
