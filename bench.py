@@ -126,25 +126,54 @@ def _one_plane(pa, vis_host, sample_M: int):
     """The bounded oracle sample: the first `sample_M` visibilities imaged through ONE w-plane of the
     configuration's mesh (same N, support, sigma, dl; the plan's whole w range mapped to a single plane), by
     the oracle's own whole-path call as it stands.  Its per-visibility stages (keys, gridding) scale with M,
-    its per-plane stages (FFT, w-correction) with the plane count.  -> (stage seconds, n_kept, wall s, threads)"""
+    its per-plane stages (FFT, w-correction) with the plane count.
+    -> (stage seconds, n_kept, wall s, threads, the oracle's image of the sample)"""
     from oracle import rick_oracle as O
     u, v, w, vv, wt = (a[:sample_M] for a in vis_host)
     pa1 = dict(pa, Nw=1)
     t0 = time.perf_counter()
-    _, n_kept, st = O.image(O.Plan(**pa1), u, v, w, vv, wt, return_timing=True)
+    img, n_kept, st = O.image(O.Plan(**pa1), u, v, w, vv, wt, return_timing=True)
     total = time.perf_counter() - t0
-    return st, n_kept, total, O.threads()
+    return st, n_kept, total, O.threads(), img
 
 
-def cpu_baseline(cfg, vis_host, pa, M: int, n_kept: int, sample_M: int = 1_000_000):
+def _sample_parity(pa, vis_host, sample_M: int, oracle_img, oracle_kept: int, gpu_image, dtype: str):
+    """Parity record of the bench line: the CUDA path, configured as the timed run (fusion mode, rick_bin mode,
+    gridding kernel), images the oracle's bounded sample (one w-plane of the configuration's mesh) and is compared
+    with the oracle image through the two gates of DESIGN.md "Parity gate".  (The whole workload against the whole
+    oracle image is tests/test_gpu_full_configs.py: minutes of oracle time.)"""
+    import numpy as np
+    from oracle import rick_oracle as O
+    img, kept = gpu_image(dict(pa, Nw=1), [a[:sample_M] for a in vis_host])
+    N = pa["N"]
+    t = O.taper(N, pa["support"], pa["sigma"], pa.get("kernel", "gauss"), pa.get("beta", 0.0))
+    tt = t / t[N // 2]
+    inner = slice(N // 4, 3 * N // 4)
+    peak = float(np.abs(oracle_img[inner, inner]).max())
+    a = b = 0.0
+    for q0 in range(0, N, 512):                       # row blocks keep the temporaries small
+        tw = np.outer(tt[q0:q0 + 512], tt)
+        d = np.abs(img[q0:q0 + 512] - oracle_img[q0:q0 + 512])
+        b = max(b, float((d * tw).max()))
+        m = tw >= 1e-2
+        if m.any():
+            a = max(a, float(d[m].max()))
+    tol = 1e-10 if dtype == "c128" else 1e-5
+    return {"against": "oracle", "sample": f"first {sample_M} visibilities through one {N}^2 plane (the cpu_baseline sample)",
+            "gate_a": a / peak, "gate_b": b / peak, "tol": tol, "n_kept_equal": bool(kept == oracle_kept),
+            "ok": bool(kept == oracle_kept and a <= tol * peak and b <= tol * peak)}
+
+
+def cpu_baseline(cfg, vis_host, pa, M: int, n_kept: int, sample_M: int = 1_000_000, gpu_image=None):
     """The oracle timed on a bounded sample (see _one_plane); the whole-workload time is estimated as
     per-visibility stages x M / M_sample + per-plane stages x Nw.  Same numerator as the GPU line (kept
     visibilities)."""
     sample_M = min(M, sample_M)
-    st, n_kept_s, total, threads = _one_plane(pa, vis_host, sample_M)
+    st, n_kept_s, total, threads, oracle_img = _one_plane(pa, vis_host, sample_M)
     scale = M / sample_M
     est = (st["keys"] + st["grid"]) * scale + (st["fft"] + st["wcorrect"]) * pa["Nw"]
-    return {
+    parity = _sample_parity(pa, vis_host, sample_M, oracle_img, n_kept_s, gpu_image, cfg.dtype) if gpu_image else None
+    return parity, {
         "value": n_kept / est, "unit": UNIT, "cores": threads, "kind": "oracle",
         "sample": (f"first {sample_M} of {M} visibilities through one of the {pa['Nw']} planes of the {pa['N']}^2 mesh: "
                    f"keys+grid {st['keys'] + st['grid']:.2f} s scaled x{scale:.1f}, fft {st['fft']:.2f} s and "
@@ -170,7 +199,7 @@ def run_reference(args):
     times = []
     last = None
     for i in range(args.warmup + args.steps):
-        st, n_kept, total, threads = _one_plane(pa, host, sample_M)
+        st, n_kept, total, threads, _ = _one_plane(pa, host, sample_M)
         if i >= args.warmup:
             times.append(total)
         last = (st, n_kept, threads)
@@ -432,7 +461,23 @@ def main():
     }
     if world == 1 and not args.no_cpu_baseline:
         opa = dict(pa, kernel=args.kernel, beta=2.34 * cfg.support if args.kernel == "kb" else 0.0)
-        line["cpu_baseline"] = cpu_baseline(cfg, [h.numpy() for h in host], opa, M, n_kept)
+        fused, sorted_outputs = int(im.fused), bool(im.sorted_outputs)
+        im.close()               # the timed plan's buffers make room for the one-plane plan of the parity sample
+        del im
+        torch.cuda.empty_cache()
+
+        def gpu_image(pa1, hv):
+            """the library, configured as the timed run, on the oracle's sample -> (host image, n_kept)"""
+            kw = {k: x for k, x in pa1.items() if k not in ("kernel", "beta")}
+            im1 = B.Imager(dtype=cfg.dtype, M_max=len(hv[0]), fused=fused, kernel=args.kernel, beta=2.34 * cfg.support,
+                           sorted_outputs=sorted_outputs, **kw)
+            assert im1.fused == fused
+            img = im1.run(*(torch.from_numpy(a).to(dev) for a in hv)).cpu().numpy()
+            kept = int(im1.n_kept.item())
+            im1.close()
+            return img, kept
+
+        line["parity"], line["cpu_baseline"] = cpu_baseline(cfg, [h.numpy() for h in host], opa, M, n_kept, gpu_image=gpu_image)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -43,6 +43,11 @@ template <> RICK_DI double2 ldg_stream<double2>(const double2* p) {
     return r;
 }
 
+// asks the L2 for `bytes` (a multiple of 16) at p: no register, no completion to wait for
+RICK_DI void prefetch_l2(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 template <typename C2, int N1, int N2>
 __global__ void __launch_bounds__(RowBig<C2, N1, N2>::T, RowBig<C2, N1, N2>::kMinBlocks)
 k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* __restrict__ list,
@@ -89,6 +94,10 @@ k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* 
     fetch(blockIdx.x);
     for (int r = blockIdx.x; r < n; r += gridDim.x) {
         C2* x = planes + (size_t)list[r] * N;
+        // the row after this one travels from DRAM to the L2 while this one is transformed: the loads at the end of
+        // the loop body then wait for the L2 only (one warp asks, 1/32 of the row per lane)
+        if (tid < 32 && r + (int)gridDim.x < n)
+            prefetch_l2(planes + (size_t)__ldg(list + r + gridDim.x) * N + tid * (N / 32), (unsigned)(sizeof(C2) * (N / 32)));
         // ---- step 1, pass 1
 #pragma unroll
         for (int i = 0; i < 32 / Ra1; ++i) {
