@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
                                                                const uint32_t* __restrict__ digit_base,
                                                                unsigned long long* __restrict__ status,
                                                                uint32_t* __restrict__ ticket, uint32_t epoch,
-                                                               GatherOut go) {
+                                                               GatherOut go, uint32_t ahead) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem<kBits>& sm = *reinterpret_cast<SortSmem<kBits>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -243,6 +243,16 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
     __syncthreads();
     const uint32_t tile = sm.tile;
     const long long tile_base = (long long)tile * kSortTile;
+    // the tile a CTA will take `ahead` tickets from now (about one wave of resident CTAs) starts its way from DRAM
+    // to the L2: 8 lanes x 4 KB of keys (and of indices)
+    if (tid < 8) {
+        const long long pf = ((long long)tile + ahead) * kSortTile;
+        if (pf + kSortTile <= M) {
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(key_in + pf + tid * (kSortTile / 8)), "r"(kSortTile / 8 * 4) : "memory");
+            if (!kFirst)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(idx_in + pf + tid * (kSortTile / 8)), "r"(kSortTile / 8 * 4) : "memory");
+        }
+    }
     const long long base = tile_base + (long long)warp * (kSortItems * 32) + lane;
     constexpr uint32_t mask = (1u << kBits) - 1u;
     constexpr int kDigitsPerThread = (1 << kBits) / kSortThreads;   // 2 (9-bit digits) or 1 (8-bit digits)
@@ -542,7 +552,8 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
                                       : (nine ? k_onesweep<false, 9, false> : k_onesweep<false, 8, false>));
             kern<<<n_tiles, kSortThreads, nine ? sizeof(SortSmem<9>) : sizeof(SortSmem<8>), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
                                                                  ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
-                                                                 (uint32_t)(pass + 1), go);
+                                                                 (uint32_t)(pass + 1), go,
+                                                                 (uint32_t)(p->sm_count * ((nine || gath) ? 2 : 3)));
             RICK_LAUNCH_CHECK();
             p->launches++;
             if (gath) break;
