@@ -26,7 +26,8 @@
  *     enqueued asynchronously on it unless stated otherwise.
  *   - Geometry [D1]: du = 1/(N dl).  Mesh node i <-> u = (i - N/2) du; pixel p <-> l = (p - N/2) dl.
  *   - Layouts: mesh grid[k][j][i], i (u) fastest, interleaved (re, im), float2 (RICK_C64) or double2
- *     (RICK_C128); image[q][p], p (l) fastest, q <-> m, fp64.
+ *     (RICK_C128), 16-byte aligned (RICK_EINVAL otherwise: 16-byte reductions and bulk copies);
+ *     image[q][p], p (l) fastest, q <-> m, fp64.
  *   - Modulated mesh: rick_grid stores (-1)^(i+j) * V~(u_i, v_j, w_k) and rick_wcorrect_accumulate
  *     applies (-1)^(p+q); with the plain (un-shifted) cuFFT in between this equals the centred
  *     transform of D7 exactly (sign flips only, N even).  A caller comparing the mesh with Eq. 3 must
@@ -94,8 +95,11 @@ int rick_plan_set_dtype(rick_plan* plan, int dtype);
  * Errors: RICK_EINVAL (unknown kind, beta <= 0 or > 64), RICK_ENOMEM, RICK_ECUDA. */
 int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
 
-/* Fused column transform (optional; RICK_C64, N in {256, 512, 1024, 2048} and |w| < 2^28 wavelengths only, RICK_EINVAL otherwise;
- * call after rick_plan_set_dtype, which switches it off, and before rick_bin).
+/* Fused column transform (optional; N a power of two, 256 <= N <= 16384, either mesh dtype, and on the fp32 mesh
+ * |w| < 2^28 wavelengths; RICK_EINVAL otherwise; call after rick_plan_set_dtype, which switches it off, and before
+ * rick_bin).  RICK_C64 with N <= 2048 uses the one-sweep kernel (whole column blocks in shared memory); larger N and
+ * RICK_C128 use the split engine: rick_fft_planes also runs the first half of the column transform in place, and
+ * rick_wcorrect_accumulate the second half.
  * on = 1: rick_fft_planes runs only the row transforms of D7 (the mesh then holds row-transformed planes),
  * and rick_wcorrect_accumulate performs the column transforms itself, fused with the phase screen, the plane
  * sum and the taper division, in one read of the mesh [D7, D8]; the image is the same within fp32 round-off.

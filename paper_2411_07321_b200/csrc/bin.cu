@@ -20,6 +20,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 32;
 constexpr int kSortTile = kSortThreads * kSortItems;   // 8192 keys per tile
 constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortAhead = 48;     // tickets between a tile and the one whose input it sends on its way to the L2
 
 struct SortLayout {
     int n_pass;
@@ -243,8 +244,10 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
     __syncthreads();
     const uint32_t tile = sm.tile;
     const long long tile_base = (long long)tile * kSortTile;
-    // the tile a CTA will take `ahead` tickets from now (about one wave of resident CTAs) starts its way from DRAM
-    // to the L2: 8 lanes x 4 KB of keys (and of indices)
+    // the tile a CTA will take `ahead` tickets from now starts its way from DRAM to the L2: 8 lanes x 4 KB of keys
+    // (and of indices).  Any distance from 8 to 110 tickets measures the same (hotspot: 21.9 -> 19.6 ms for the four
+    // passes); a whole wave of resident CTAs (444) is too far: the lines are evicted before use (13.1 instead of
+    // 8.2 GB of DRAM reads per pass).
     if (tid < 8) {
         const long long pf = ((long long)tile + ahead) * kSortTile;
         if (pf + kSortTile <= M) {
@@ -553,7 +556,7 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
             kern<<<n_tiles, kSortThreads, nine ? sizeof(SortSmem<9>) : sizeof(SortSmem<8>), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
                                                                  ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
                                                                  (uint32_t)(pass + 1), go,
-                                                                 (uint32_t)(p->sm_count * ((nine || gath) ? 2 : 3)));
+                                                                 (uint32_t)kSortAhead);
             RICK_LAUNCH_CHECK();
             p->launches++;
             if (gath) break;

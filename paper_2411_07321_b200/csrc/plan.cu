@@ -437,7 +437,7 @@ int rick_bin(rick_plan* p, long long M, const float* u, const float* v, const fl
 }
 
 int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
-    if (!p || !grid) return RICK_EINVAL;
+    if (!p || !grid || ((uintptr_t)grid & 15)) return RICK_EINVAL;     // 16-byte reductions, bulk copies
     if (!p->bound) return RICK_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (p->fused == 2) {          // clear only the rows the bound visibilities touch and that are not defined yet
@@ -454,7 +454,7 @@ int rick_grid(rick_plan* p, void* grid, int zero_first, void* stream) {
 }
 
 int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_bytes, void* stream) {
-    if (!p || !grid) return RICK_EINVAL;
+    if (!p || !grid || ((uintptr_t)grid & 15)) return RICK_EINVAL;
     if (!p->fft_ready) return RICK_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (p->fused == 2 && !p->split) {   // row transforms of the defined rows only, by the library's own kernel (colfft.cu)
@@ -518,7 +518,7 @@ int rick_fft_planes(rick_plan* p, void* grid, void* fft_work, size_t fft_work_by
 }
 
 int rick_wcorrect_accumulate(rick_plan* p, const void* grid, double* image, int zero_first, void* stream) {
-    if (!p || !grid || !image) return RICK_EINVAL;
+    if (!p || !grid || !image || ((uintptr_t)grid & 15) || ((uintptr_t)image & 7)) return RICK_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     StageTimer tm(p, RICK_T_WCORRECT, st);
     if (p->fused && p->split) return rick_colsplit_b_impl(p, grid, image, zero_first, st);
