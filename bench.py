@@ -324,6 +324,8 @@ def main():
     rows_total = cfg.Nw * cfg.N
     rows_defined = B.rick_plan_rows_defined(im.plan) if im.fused == 2 else rows_total
     live_bytes = mesh_bytes * rows_defined // rows_total
+    # where the long-row kernel runs, clearing and the row transform's reads are by segment of a row (rows.cu)
+    seg_bytes = B.rick_plan_cells_defined(im.plan) * cell if im.fused == 2 else mesh_bytes
     one_sweep = bool(im.fused) and cfg.dtype == "c64" and cfg.N <= 2048      # colfft.cu; else the split engine (colsplit.cu)
     split = bool(im.fused) and not one_sweep
     if not im.fused:
@@ -333,7 +335,7 @@ def main():
         col_a_b, fft_b, wc_b = 0, fft_rows_b, live_bytes + cfg.N * cfg.N * 8
     else:
         own_rows = im.fused == 2 and cfg.N >= 4096 and not (cfg.dtype == "c128" and cfg.N > 8192)   # rowbig.cu
-        fft_rows_b = 2 * live_bytes if own_rows else 2 * mesh_bytes      # else batched library transforms of every row
+        fft_rows_b = seg_bytes + live_bytes if own_rows else 2 * mesh_bytes      # reads the defined segments, writes the defined rows; else batched library transforms of every row
         col_a_b = live_bytes + mesh_bytes    # sweep A reads the defined rows, writes every row
         fft_b, wc_b = fft_rows_b + col_a_b, mesh_bytes + cfg.N * cfg.N * 8
     indirect = not im.sorted_outputs    # fp32 mesh: rick_bin gathers nothing; the gridder fetches 32-B records by index
@@ -345,7 +347,7 @@ def main():
         # and one 32-B record per kept visibility)
         "sort": ((12 + 16 * (n_pass - 1)) * M if indirect else
                  ((12 if n_pass > 1 else 4) + 16 * max(n_pass - 2, 0) + (8 if n_pass > 1 else 0)) * M + (32 + 48) * n_kept),
-        "zero": live_bytes if im.fused == 2 else mesh_bytes,
+        "zero": seg_bytes if im.fused == 2 else mesh_bytes,
         "grid": (4 + 32) * n_kept if indirect else 24 * n_kept,
         "fft": fft_b, "fft_rows": fft_rows_b, "fft_col_a": col_a_b,
         "wcorrect": wc_b,
@@ -450,7 +452,7 @@ def main():
                    "support": cfg.support, "sigma": cfg.sigma, "gridding_kernel": args.kernel, "mesh": cfg.dtype,
                    "fusion_mode": int(im.fused), "rick_bin_sorted_outputs": bool(im.sorted_outputs),
                    "column_engine": "split (colsplit.cu)" if split else ("one sweep (colfft.cu)" if one_sweep else "cuFFT 2-D + K5"),
-                   "mesh_rows_defined": rows_defined, "mesh_rows": rows_total,
+                   "mesh_rows_defined": rows_defined, "mesh_rows": rows_total, "mesh_bytes_defined_before_fft": seg_bytes,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs ({24 * M / 1e9:.2f} GB) and mesh ({mesh_bytes / 1e9:.2f} GB) exceed the 126 MB L2; no explicit flush"},
         "value_definition": "kept (gridded) visibilities of all ranks / step time; a step = rick_bin + rick_grid + rick_fft_planes + rick_wcorrect_accumulate",

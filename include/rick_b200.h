@@ -105,13 +105,21 @@ int rick_plan_set_kernel(rick_plan* plan, int kind, double param);
  * sum and the taper division, in one read of the mesh [D7, D8]; the image is the same within fp32 round-off.
  * on = 2: in addition the library tracks which mesh rows (plane, j) some footprint touches: rick_grid clears
  * only touched rows that are not defined yet (instead of the whole mesh) and the fused kernel reads only
- * defined rows; mesh rows no footprint touches then hold UNDEFINED data (only the image is an output).
+ * defined rows; mesh rows no footprint touches then hold UNDEFINED data (only the image is an output).  Where the
+ * library's own long-row kernel runs (N >= 4096; RICK_C128: N <= 8192) the same holds per segment of a row
+ * (64 segments of N / 64 cells): only touched segments are cleared and read, the rest of a touched row is
+ * undefined between rick_grid and rick_fft_planes as well.
  * on = 0: off. */
 int rick_plan_set_fusion(rick_plan* plan, int on);
 
 /* Fusion mode 2 only: number of mesh rows (plane, j) that held defined data at the last rick_fft_planes
  * (of Nw * N).  Host-synchronous.  RICK_ESTATE in other modes. */
 int rick_plan_rows_defined(rick_plan* plan, long long* rows);
+
+/* Fusion mode 2 only: number of mesh cells that hold defined data since the last rick_grid(zero_first != 0) -- the
+ * cells of the defined segments, or of the defined rows where rows are the unit.  Host-synchronous (copies the
+ * segment masks to the host).  RICK_ESTATE in other modes. */
+int rick_plan_cells_defined(rick_plan* plan, long long* cells);
 
 /* Sizes of the two caller-provided scratch buffers: `bin_bytes` for rick_bin with up to M
  * visibilities, `fft_bytes` for rick_fft_planes (0 if cuFFT needs none).  Either pointer may be NULL. */

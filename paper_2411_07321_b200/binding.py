@@ -24,7 +24,7 @@ EXPORTS = (
     "rick_plan_sort_layout", "rick_plan_set_fusion", "rick_plan_set_kernel", "rick_plan_rows_defined",
     "rick_bin", "rick_grid", "rick_fft_planes", "rick_wcorrect_accumulate", "rick_image",
     "rick_image_from_host", "rick_image_from_host_chunked", "rick_get_timings", "rick_launch_count", "rick_strerror",
-    "rick_measure_fp32_rate", "rick_measure_random_read_rate", "rick_bin_static",
+    "rick_measure_fp32_rate", "rick_measure_random_read_rate", "rick_bin_static", "rick_plan_cells_defined",
 )
 
 
@@ -65,6 +65,7 @@ def lib():
         L.rick_plan_set_fusion.argtypes = [vp, i]
         L.rick_plan_set_kernel.argtypes = [vp, i, dbl]
         L.rick_plan_rows_defined.argtypes = [vp, C.POINTER(ll)]
+        L.rick_plan_cells_defined.argtypes = [vp, C.POINTER(ll)]
         L.rick_plan_sort_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.rick_bin.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, sz, vp, vp]
         L.rick_bin_static.argtypes = [vp, ll] + [vp] * 5 + [vp] * 5 + [vp, vp, vp, vp, vp]
@@ -149,6 +150,13 @@ def rick_plan_rows_defined(plan: int) -> int:
     """Fusion mode 2: mesh rows that held defined data at the last rick_fft_planes."""
     n = C.c_longlong()
     _check(lib().rick_plan_rows_defined(plan, C.byref(n)), "rick_plan_rows_defined")
+    return int(n.value)
+
+
+def rick_plan_cells_defined(plan: int) -> int:
+    """Fusion mode 2: mesh cells that hold defined data (defined segments, or defined rows where rows are the unit)."""
+    n = C.c_longlong()
+    _check(lib().rick_plan_cells_defined(plan, C.byref(n)), "rick_plan_cells_defined")
     return int(n.value)
 
 

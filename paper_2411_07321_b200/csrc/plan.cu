@@ -335,7 +335,7 @@ int rick_plan_set_kernel(rick_plan* p, int kind, double param) {
 int rick_plan_set_fusion(rick_plan* p, int on) {
     if (!p) return RICK_EINVAL;
     if (on < 0 || on > 2) return RICK_EINVAL;
-    if (!on) { p->fused = 0; return RICK_OK; }
+    if (!on) { p->fused = 0; p->segs = false; return RICK_OK; }
     if (!p->dtype_set) return RICK_ESTATE;
     // engine: the one-sweep column kernel where a column block fits one SM (fp32 mesh, N <= 2048), else the
     // split column transform (two sweeps; N up to 16384, both mesh types)
@@ -357,7 +357,41 @@ int rick_plan_set_fusion(rick_plan* p, int on) {
         RICK_CUDA(cudaMemset(p->occ_cur_dev, 0, 4 * words));
         RICK_CUDA(cudaMemset(p->occ_mesh_dev, 0, 4 * words));
     }
+    // segment occupancy: where the library's own long-row kernel transforms the rows (it takes zeros for the
+    // segments of a row no footprint touches)
+    p->segs = (on == 2) && p->split && rick_rowbig_supported(p);
+    if (p->segs && !p->seg_cur_dev) {
+        const size_t rows = (size_t)p->g.Nw * p->g.N;
+        if (cudaMalloc((void**)&p->seg_cur_dev, 8 * rows) != cudaSuccess ||
+            cudaMalloc((void**)&p->seg_mesh_dev, 8 * rows) != cudaSuccess ||
+            cudaMalloc((void**)&p->seg_fresh_dev, 8 * rows) != cudaSuccess)
+            return RICK_ENOMEM;
+        RICK_CUDA(cudaMemset(p->seg_cur_dev, 0, 8 * rows));
+        RICK_CUDA(cudaMemset(p->seg_mesh_dev, 0, 8 * rows));
+        RICK_CUDA(cudaMemset(p->seg_fresh_dev, 0, 8 * rows));
+    }
     p->fused = on;
+    return RICK_OK;
+}
+
+int rick_plan_cells_defined(rick_plan* p, long long* cells) {
+    if (!p || !cells) return RICK_EINVAL;
+    if (p->fused != 2 || !p->n_rows_dev) return RICK_ESTATE;
+    RICK_CUDA(cudaDeviceSynchronize());
+    if (!p->segs) {
+        uint32_t n = 0;
+        RICK_CUDA(cudaMemcpy(&n, p->n_rows_dev, sizeof(n), cudaMemcpyDeviceToHost));
+        *cells = (long long)n * p->g.N;
+        return RICK_OK;
+    }
+    const size_t rows = (size_t)p->g.Nw * p->g.N;
+    unsigned long long* h = (unsigned long long*)malloc(8 * rows);
+    if (!h) return RICK_ENOMEM;
+    if (cudaMemcpy(h, p->seg_mesh_dev, 8 * rows, cudaMemcpyDeviceToHost) != cudaSuccess) { free(h); return RICK_ECUDA; }
+    long long n = 0;
+    for (size_t r = 0; r < rows; ++r) n += __builtin_popcountll(h[r]);
+    free(h);
+    *cells = n * (p->g.N / 64);
     return RICK_OK;
 }
 
@@ -402,6 +436,9 @@ int rick_plan_destroy(rick_plan* p) {
     if (p->occ_mesh_dev) cudaFree(p->occ_mesh_dev);
     if (p->row_list_dev) cudaFree(p->row_list_dev);
     if (p->n_rows_dev) cudaFree(p->n_rows_dev);
+    if (p->seg_cur_dev) cudaFree(p->seg_cur_dev);
+    if (p->seg_mesh_dev) cudaFree(p->seg_mesh_dev);
+    if (p->seg_fresh_dev) cudaFree(p->seg_fresh_dev);
     if (p->kb_lut_f_dev) cudaFree(p->kb_lut_f_dev);
     if (p->kb_lut_d_dev) cudaFree(p->kb_lut_d_dev);
     for (int i = 0; i < RICK_T_COUNT; ++i) {

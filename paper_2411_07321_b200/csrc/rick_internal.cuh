@@ -61,6 +61,12 @@ struct rick_plan {
     uint32_t *occ_cur_dev, *occ_mesh_dev;
     uint32_t* row_list_dev;  // [Nw N] rows to clear, built by rick_grid
     uint32_t* n_rows_dev;
+    // segment occupancy (mode 2 with the library's own long-row kernel, rowbig.cu): a mesh row is 64 segments of
+    // N / 64 cells; bit s of seg_cur[k N + j] = segment s of that row is touched by a footprint of the bound
+    // visibilities, seg_mesh = it holds defined data, seg_fresh = it is cleared by the rick_grid in progress.
+    // Only defined segments are cleared and read by the row transform (which writes whole rows).
+    bool segs;
+    unsigned long long *seg_cur_dev, *seg_mesh_dev, *seg_fresh_dev;
     cufftHandle fft_rows;    // batched 1-D row transforms
     bool fft_rows_ready;
     size_t fft_rows_work_bytes;

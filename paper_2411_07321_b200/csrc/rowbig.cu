@@ -11,6 +11,9 @@
 // writes 32 consecutive frequencies q1 + N1 q2.
 // A thread holds 32 elements; the twiddles W_N^(j2 q1) of its elements do not depend on the row: W_N^(j2 u) per
 // butterfly and the powers of W_N^(j2 R1) stay in registers for all rows of the CTA.
+// Segment occupancy (rows.cu): of a listed row only the segments (N / 64 cells each) some footprint touched hold
+// defined data; the others are not read (nor prefetched) and count as zeros.  A segment is N1 / 64 whole lines j1 of
+// the matrix, so the test is uniform over a warp.  The row is written whole.
 #include "fft_radix.cuh"
 #include "rick_internal.cuh"
 
@@ -31,15 +34,22 @@ template <typename C2, int N1, int N2> struct RowBig {
     static constexpr int kMinBlocks = kBySmem < kByRegs ? (kBySmem < 1 ? 1 : kBySmem) : (kByRegs < 1 ? 1 : kByRegs);
 };
 
-template <typename C2> RICK_DI C2 ldg_stream(const C2* p);
-template <> RICK_DI float2 ldg_stream<float2>(const float2* p) {
+// streaming load of one complex value when `live`, else zero -- predicated, no branch
+template <typename C2> RICK_DI C2 ldg_stream_if(const C2* p, bool live);
+template <> RICK_DI float2 ldg_stream_if<float2>(const float2* p, bool live) {
     float2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+                 "mov.f32 %0, 0f00000000;\n\tmov.f32 %1, 0f00000000;\n\t"
+                 "@q ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];\n\t}"
+                 : "=&f"(r.x), "=&f"(r.y) : "l"(p), "r"((unsigned)live));
     return r;
 }
-template <> RICK_DI double2 ldg_stream<double2>(const double2* p) {
+template <> RICK_DI double2 ldg_stream_if<double2>(const double2* p, bool live) {
     double2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+                 "mov.f64 %0, 0d0000000000000000;\n\tmov.f64 %1, 0d0000000000000000;\n\t"
+                 "@q ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];\n\t}"
+                 : "=&d"(r.x), "=&d"(r.y) : "l"(p), "r"((unsigned)live));
     return r;
 }
 
@@ -51,11 +61,13 @@ RICK_DI void prefetch_l2(const void* p, unsigned bytes) {
 template <typename C2, int N1, int N2>
 __global__ void __launch_bounds__(RowBig<C2, N1, N2>::T, RowBig<C2, N1, N2>::kMinBlocks)
 k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* __restrict__ list,
-          const uint32_t* __restrict__ n_rows) {
+          const uint32_t* __restrict__ n_rows, const unsigned long long* __restrict__ seg) {
     typedef RowBig<C2, N1, N2> P;
     constexpr int N = P::N, T = P::T, PB = P::PB;
     constexpr int Ra1 = Split<N1>::R1, Ra2 = Split<N1>::R2, Rb1 = Split<N2>::R1, Rb2 = Split<N2>::R2;
     static_assert(T % N2 == 0 && T % N1 == 0, "a thread keeps its j2 (step 1) and its q1 (step 2) for all butterflies");
+    static_assert(N1 % 64 == 0 && N2 % 32 == 0, "a segment (N / 64 cells) is N1 / 64 whole lines j1, and a warp stays within one line");
+    constexpr int kSegLines = N1 / 64;                                // lines j1 per segment
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C2* buf = reinterpret_cast<C2*>(smem_raw);
     C2* twA = buf + P::elems;           // W_N1^i
@@ -82,22 +94,42 @@ k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* 
     // the inputs of the first pass (radix Ra1 over j1 = m + t Ra2) come straight from global memory; the next row's
     // are requested as soon as this row's last butterflies have left the registers, before the closing barrier
     C2 v[32];
-    auto fetch = [&](int r) {
-        const C2* x = planes + (size_t)__ldg(list + r) * N;
+    auto fetch = [&](uint32_t row, unsigned long long segs) {
+        const C2* x = planes + (size_t)row * N;
 #pragma unroll
         for (int i = 0; i < 32 / Ra1; ++i) {
             const int m = a0 + i * aStep;
 #pragma unroll
-            for (int t = 0; t < Ra1; ++t) v[i * Ra1 + t] = ldg_stream(x + (m + t * Ra2) * N2 + j2);
+            for (int t = 0; t < Ra1; ++t) {
+                const int j1 = m + t * Ra2;
+                v[i * Ra1 + t] = ldg_stream_if(x + j1 * N2 + j2, (segs >> (j1 / kSegLines)) & 1ull);
+            }
         }
     };
-    fetch(blockIdx.x);
-    for (int r = blockIdx.x; r < n; r += gridDim.x) {
-        C2* x = planes + (size_t)list[r] * N;
-        // the row after this one travels from DRAM to the L2 while this one is transformed: the loads at the end of
-        // the loop body then wait for the L2 only (one warp asks, 1/32 of the row per lane)
-        if (tid < 32 && r + (int)gridDim.x < n)
-            prefetch_l2(planes + (size_t)__ldg(list + r + gridDim.x) * N + tid * (N / 32), (unsigned)(sizeof(C2) * (N / 32)));
+    // row numbers and segment masks run one row ahead of the loads, which run one row ahead of the arithmetic
+    const int G = (int)gridDim.x;
+    uint32_t row_cur = __ldg(list + blockIdx.x), row_nxt = 0;
+    unsigned long long m_nxt = 0;
+    if ((int)blockIdx.x + G < n) {
+        row_nxt = __ldg(list + blockIdx.x + G);
+        m_nxt = seg ? __ldg(seg + row_nxt) : ~0ull;
+    }
+    fetch(row_cur, seg ? __ldg(seg + row_cur) : ~0ull);
+    for (int r = blockIdx.x; r < n; r += G) {
+        C2* x = planes + (size_t)row_cur * N;
+        // the defined segments of the row after this one travel from DRAM to the L2 while this one is transformed: the
+        // loads at the end of the loop body then wait for the L2 only (one warp asks, two segments per lane)
+        if (tid < 32 && r + G < n) {
+            const C2* xn = planes + (size_t)row_nxt * N + (size_t)tid * (N / 32);
+            if ((m_nxt >> (2 * tid)) & 1ull) prefetch_l2(xn, (unsigned)(sizeof(C2) * (N / 64)));
+            if ((m_nxt >> (2 * tid + 1)) & 1ull) prefetch_l2(xn + N / 64, (unsigned)(sizeof(C2) * (N / 64)));
+        }
+        uint32_t row_n2 = 0;
+        unsigned long long m_n2 = 0;
+        if (r + 2 * G < n) {
+            row_n2 = __ldg(list + r + 2 * G);
+            m_n2 = seg ? __ldg(seg + row_n2) : ~0ull;
+        }
         // ---- step 1, pass 1
 #pragma unroll
         for (int i = 0; i < 32 / Ra1; ++i) {
@@ -149,8 +181,11 @@ k_row_big(C2* __restrict__ planes, const C2* __restrict__ tw_g, const uint32_t* 
 #pragma unroll
             for (int s = 0; s < Rb2; ++s) x[q1 + N1 * (u + Rb1 * s)] = v[i * Rb2 + s];
         }
-        if (r + (int)gridDim.x < n) fetch(r + (int)gridDim.x);
+        if (r + G < n) fetch(row_nxt, m_nxt);
         __syncthreads();                         // the buffer is free for the next row
+        row_cur = row_nxt;
+        row_nxt = row_n2;
+        m_nxt = m_n2;
     }
 }
 
@@ -165,7 +200,8 @@ int launch_row_big(rick_plan* p, void* grid, cudaStream_t st) {
         done = true;
     }
     const int ctas = p->sm_count * P::kMinBlocks;       // persistent: every CTA walks its share of the row list
-    k_row_big<C2, N1, N2><<<ctas, P::T, P::smem, st>>>((C2*)grid, (const C2*)p->split_tw, p->row_list_dev, p->n_rows_dev);
+    k_row_big<C2, N1, N2><<<ctas, P::T, P::smem, st>>>((C2*)grid, (const C2*)p->split_tw, p->row_list_dev, p->n_rows_dev,
+                                                       p->segs ? p->seg_mesh_dev : nullptr);
     return RICK_OK;
 }
 
