@@ -48,13 +48,15 @@ __device__ __forceinline__ void mark_rows(const RickGeom& g, uint32_t j0, uint32
                                           unsigned long long* __restrict__ seg, int seg_shift) {
     const uint32_t lo = k * (uint32_t)g.N + (j0 - (uint32_t)g.h), hi = lo + 2u * (uint32_t)g.h;
     if (seg) {
-        // the footprints of the visibilities of tile column tx lie in columns 32 tx - h .. 32 tx + 31 + h: one or
-        // two segments (a segment is at least 64 cells wide), marked in every row j0 - h .. j0 + h
+        // segment mode: the footprints of the visibilities of tile column tx lie in columns 32 tx - h .. 32 tx + 31 + h:
+        // one or two segments (a segment is at least 64 cells wide), marked on the CENTRE row j0 only; k_segs_dilate
+        // spreads them over j0 - h .. j0 + h afterwards, and the row bitmap follows from the masks (k_segs_new)
         const int c_lo = (int)(tx * 32u) - g.h, c_hi = (int)(tx * 32u) + 31 + g.h;
         const int s_lo = (c_lo < 0 ? 0 : c_lo) >> seg_shift, s_hi = (c_hi > g.N - 1 ? g.N - 1 : c_hi) >> seg_shift;
         const unsigned long long m = (1ull << s_lo) | (1ull << s_hi);
-        for (uint32_t r = lo; r <= hi; ++r)
-            if ((__ldcg(seg + r) & m) != m) atomicOr(seg + r, m);
+        unsigned long long* c = seg + (k * (uint32_t)g.N + j0);
+        if ((__ldcg(c) & m) != m) atomicOr(c, m);
+        return;
     }
     const uint32_t w0 = lo >> 5, w1 = hi >> 5;
     const uint32_t span = (2u * (uint32_t)g.h + 1u);
@@ -162,6 +164,20 @@ __global__ void __launch_bounds__(256) k_rows_zero(const uint32_t* __restrict__ 
     }
 }
 
+// Segment mode: cur[r] = OR of the centre-row masks c0[r - h .. r + h] (rows j0 < h and j0 > N - 1 - h are never
+// centres, D5, so nothing leaks across a plane boundary)
+__global__ void __launch_bounds__(256) k_segs_dilate(int n_rows, int h, const unsigned long long* __restrict__ c0,
+                                                     unsigned long long* __restrict__ cur) {
+    const int r = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+    if (r >= n_rows) return;
+    unsigned long long m = 0;
+    for (int d = -h; d <= h; ++d) {
+        const int q = r + d;
+        if (q >= 0 && q < n_rows) m |= __ldg(c0 + q);
+    }
+    cur[r] = m;
+}
+
 // Segment mode.  One warp per 32 rows: rows with a touched segment that is not defined yet go on the list, with the
 // mask of those segments in seg_fresh; seg_mesh |= seg_cur; the row bitmap occ_mesh |= "some segment touched".
 __global__ void __launch_bounds__(256) k_segs_new(int n_words, const unsigned long long* __restrict__ seg_cur,
@@ -212,11 +228,16 @@ __global__ void __launch_bounds__(256) k_segs_zero(const uint32_t* __restrict__ 
 int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
     const size_t words = (size_t)p->g.Nw * p->g.N / 32;
     RICK_CUDA(cudaMemsetAsync(p->occ_cur_dev, 0, 4 * words, st));
-    unsigned long long* seg = p->segs ? p->seg_cur_dev : nullptr;
+    // segment mode: centre-row masks into seg_fresh (free between two rick_grid calls), dilated into seg_cur below
+    unsigned long long* seg = p->segs ? p->seg_fresh_dev : nullptr;
+    const int n_rows = p->g.Nw * p->g.N;
     int seg_shift = 0;
     while ((64 << seg_shift) < p->g.N) ++seg_shift;                     // a segment is N / 64 = 2^seg_shift cells
-    if (seg) RICK_CUDA(cudaMemsetAsync(seg, 0, 8 * (size_t)p->g.Nw * p->g.N, st));
-    if (M == 0) return RICK_OK;
+    if (seg) RICK_CUDA(cudaMemsetAsync(seg, 0, 8 * (size_t)n_rows, st));
+    if (M == 0) {
+        if (seg) RICK_CUDA(cudaMemsetAsync(p->seg_cur_dev, 0, 8 * (size_t)n_rows, st));
+        return RICK_OK;
+    }
     const long long want = (M + 255) / 256;
     const long long cap = (long long)p->sm_count * 16;
     if (p->indirect) {
@@ -229,6 +250,11 @@ int rick_rows_mark(rick_plan* p, long long M, cudaStream_t st) {
         k_rows_mark<<<(int)(want > cap ? cap : want), 256, 0, st>>>(p->g, p->n_kept_dev, RowsFromRecords{p->grec_a}, p->occ_cur_dev, seg, seg_shift);
     RICK_LAUNCH_CHECK();
     p->launches++;
+    if (seg) {
+        k_segs_dilate<<<(n_rows + 255) / 256, 256, 0, st>>>(n_rows, p->g.h, seg, p->seg_cur_dev);
+        RICK_LAUNCH_CHECK();
+        p->launches++;
+    }
     return RICK_OK;
 }
 
