@@ -516,6 +516,46 @@ def test_split_column_transform(name, M, plan, dtype, fused):
     im.close()
 
 
+@pytest.mark.parametrize("dtype,N", [("c64", 4096), ("c128", 4096)])
+def test_segment_occupancy_accumulates_across_slices(dtype, N):
+    """Fusion mode 2 where the long-row kernel runs keeps the occupancy per SEGMENT of a mesh row (rows.cu: 64
+    segments of N / 64 cells).  A second rick_bin / rick_grid(zero_first = 0) whose visibilities fall into OTHER
+    segments of rows the first one defined (left half of the uv plane, then the right half) must clear exactly those
+    segments first: the mesh is pre-filled with NaN, the image of the two halves equals the image of the whole
+    input, and the defined cells are the same set, sparser than the defined rows."""
+    cfg, vis, pa = make("500M", 300_000, dtype=dtype, N=N, Nw=2)
+    im = B.Imager(dtype=dtype, M_max=vis.M, fused=2, **pa)
+    assert im.fused == 2
+    real = torch.float64 if dtype == "c128" else torch.float32
+    im.grid.view(real).fill_(float("nan"))
+    whole = im.run(vis.u, vis.v, vis.w, vis.vis, vis.weight).cpu().numpy().copy()
+    assert np.isfinite(whole).all()
+    rows = B.rick_plan_rows_defined(im.plan)
+    cells = B.rick_plan_cells_defined(im.plan)
+    assert 0 < cells < rows * N and cells % (N // 64) == 0          # whole segments, fewer than whole rows
+    ref = O.image(O.Plan(**pa), *vis.numpy())
+    a, b, _ = gates(whole, ref, N, cfg.support, cfg.sigma)
+    assert a <= TOL[dtype] and b <= TOL[dtype]
+    im.grid.view(real).fill_(float("nan"))
+    left = vis.u < 0
+    seen = []
+    for n, sel in enumerate((left, ~left)):
+        im.bin(*(t[sel].contiguous() for t in (vis.u, vis.v, vis.w, vis.vis, vis.weight)))
+        im.grid_(zero_first=(n == 0))
+        torch.cuda.synchronize()
+        seen.append(B.rick_plan_cells_defined(im.plan))
+    assert 0 < seen[0] < seen[1] == cells
+    im.fft()
+    im.wcorrect(True)
+    torch.cuda.synchronize()
+    halves = im.image.cpu().numpy()
+    assert np.isfinite(halves).all()
+    t = O.taper(N, cfg.support, cfg.sigma)
+    tw = np.outer(t, t) / t[N // 2] ** 2
+    assert (np.abs(halves - whole) * tw).max() <= (1e-12 if dtype == "c128" else 2e-6) * np.abs(whole * tw).max()
+    im.close()
+
+
 @pytest.mark.parametrize("S", [3, 5, 7, 9, 11, 13, 15])
 @pytest.mark.parametrize("dtype,sorted_outputs", [("c64", False), ("c64", True), ("c128", True)])
 @pytest.mark.parametrize("kernel", ["gauss", "kb"])
