@@ -527,6 +527,37 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_rec(RickGeom g, TapConst t
             __syncthreads();                    // buffer st & 1 is free for stage st + 2
         }
         }
+        // End of the ranges.  The lanes of a warp hold consecutive ranges of the sorted records, so where a hot cell
+        // spans many ranges (hotspot: 7 600 visibilities per core cell against 256 per range) neighbouring lanes end on
+        // the same window: those lanes merge their accumulators (segmented sum over the lanes) and only the last lane
+        // of a segment flushes -- one footprint of reductions per warp and hot cell instead of one per lane, all of
+        // them aimed at the same few L2 lines.  Warps whose lanes all end on different windows skip this.
+        {
+            const unsigned kFull = 0xffffffffu;
+            const int lane = tid & 31;
+            const uint32_t up_ij = __shfl_up_sync(kFull, cij, 1), up_k = __shfl_up_sync(kFull, ck, 1);
+            const bool joins = lane > 0 && cij != 0xFFFFFFFFu && up_ij == cij && up_k == ck;
+            const unsigned heads = ~__ballot_sync(kFull, joins);            // bit l: lane l starts a segment (bit 0 is set)
+            if (heads != kFull) {                                            // warp-uniform
+                const int start = 31 - __clz((int)(heads & (kFull >> (31 - lane))));   // first lane of this lane's segment
+#pragma unroll 1
+                for (int d = 1; d < 32; d <<= 1) {
+                    const bool take = lane - d >= start;
+#pragma unroll
+                    for (int r = 0; r < RB; ++r)
+#pragma unroll
+                        for (int a = 0; a < W; ++a) {
+                            const float ox = __shfl_up_sync(kFull, acc[r][a].x, d), oy = __shfl_up_sync(kFull, acc[r][a].y, d);
+                            if (take) {
+                                acc[r][a].x += ox;
+                                acc[r][a].y += oy;
+                            }
+                        }
+                }
+                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+                if (!tail) cij = 0xFFFFFFFFu;                                // its sum lives on in a later lane
+            }
+        }
         if (cij != 0xFFFFFFFFu) flush();
     }
 }
