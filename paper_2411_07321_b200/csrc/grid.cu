@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
     constexpr int W = kWin ? S + 1 : S;
     const long long n = *n_kept;
     const long long first = ((long long)blockIdx.x * kRunThreads + threadIdx.x) * L;   // L: a multiple of 4
-    if (first >= n) return;
+    if ((long long)blockIdx.x * kRunThreads * L >= n) return;      // whole block past the end (lanes past it stay for the merge)
     const size_t N = (size_t)g.N;
 
 #pragma unroll
@@ -278,6 +278,33 @@ __global__ void __launch_bounds__(kRunThreads) k_grid_runs(RickGeom g, TapConst 
             if (p + 1 < n) one(u4.y, v4.y, w4.y, va.z, va.w, t4.y);
             if (p + 2 < n) one(u4.z, v4.z, w4.z, vb.x, vb.y, t4.z);
             if (p + 3 < n) one(u4.w, v4.w, w4.w, vb.z, vb.w, t4.w);
+        }
+        // end of the ranges: lanes that end on the same cell merge their accumulators, one lane flushes (see k_grid_rec)
+        {
+            const unsigned kFull = 0xffffffffu;
+            const int lane = (int)(threadIdx.x & 31);
+            const int up_i = __shfl_up_sync(kFull, ci, 1), up_j = __shfl_up_sync(kFull, cj, 1), up_k = __shfl_up_sync(kFull, ck, 1);
+            const bool joins = lane > 0 && ci >= 0 && up_i == ci && up_j == cj && up_k == ck;
+            const unsigned heads = ~__ballot_sync(kFull, joins);
+            if (heads != kFull) {
+                const int start = 31 - __clz((int)(heads & (kFull >> (31 - lane))));
+#pragma unroll 1
+                for (int d = 1; d < 32; d <<= 1) {
+                    const bool take = lane - d >= start;
+#pragma unroll
+                    for (int r = 0; r < RB; ++r)
+#pragma unroll
+                        for (int a = 0; a < W; ++a) {
+                            const real orr = __shfl_up_sync(kFull, ar[r][a], d), oi = __shfl_up_sync(kFull, ai[r][a], d);
+                            if (take) {
+                                ar[r][a] += orr;
+                                ai[r][a] += oi;
+                            }
+                        }
+                }
+                const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+                if (!tail) ci = -1;
+            }
         }
         if (ci >= 0) flush();
     }
