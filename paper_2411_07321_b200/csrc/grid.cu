@@ -11,6 +11,9 @@
 //
 // and only when the footprint window changes (or its range ends) adds it to the mesh with reductions in
 // L2.  No shared-memory accumulation: fp32 atomicAdd on shared memory is a CAS loop on sm_100a.
+// At the end of the ranges the lanes of a warp, which hold consecutive ranges, merge the windows they share
+// (segmented sum over the lanes by shuffles) and one lane per window flushes: a hot cell spans many ranges
+// (hotspot: 7 600 visibilities per core cell), and its per-range flushes would all land on the same few L2 lines.
 //
 //   k_grid_rec  (fp32 mesh)  reads the 24-byte gridder records the gather wrote (cell, plane, fractional
 //               offsets, signed weight * V), staged through shared memory with coalesced cp.async copies;
