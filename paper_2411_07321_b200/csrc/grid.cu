@@ -4,7 +4,7 @@
 // Run-accumulating gridders.  rick_bin leaves the kept visibilities sorted by (plane, tile, cell) [D4'],
 // so visibilities that share a nearest cell (i0, j0, k) -- and therefore the same S x S footprint --
 // are adjacent: 87 % of the "10M" workload sits in runs of >= 8.
-// Each thread walks a range of consecutive sorted visibilities (32 .. 256) and keeps the whole footprint
+// Each thread walks a range of consecutive sorted visibilities (16 .. 128) and keeps the whole footprint
 // (or a block of RB rows of it per pass) in registers:
 //
 //     acc[b][a] += gx[a] * (gy[b] * weight * V)          2 FMAs per cell and visibility
@@ -613,11 +613,14 @@ int launch_rec_k(rick_plan* p, void* grid, cudaStream_t st) {
         tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
         tc.Kf[t] = (float)tc.K[t];
     }
-    // records per thread: long enough that end-of-range flushes are rare next to run ends (dense inputs
-    // put thousands of visibilities on one cell), short enough for >= ~12 CTAs per SM slot; at most 256
+    // records per thread: short ranges keep a CTA's threads on neighbouring cells (L2 locality of the reductions)
+    // and balance the CTAs; the flushes at their ends cost little since the lanes of a warp merge the windows
+    // they share.  Measured with that merge, indirect / direct mode: hotspot 32: 26.1 / --, 64: 25.7 / 17.9,
+    // 128: 26.8 / 18.2, 256: 28.1 / 18.8 ms; 500M 32: 10.9 / 8.1, 64: 10.9 / 7.4, 128: 11.6 / 7.0, 256: 12.8 / 7.0 ms.
+    constexpr int kMaxRange = kIdx ? 64 : 128;
     const long long want = p->M / ((long long)kRunThreads * p->sm_count * 2 * 12);
     int n_stage = (int)(want / L);
-    n_stage = n_stage < 2 ? 2 : (n_stage > 256 / L ? 256 / L : n_stage);
+    n_stage = n_stage < 2 ? 2 : (n_stage > kMaxRange / L ? kMaxRange / L : n_stage);
     const long long per_block = (long long)kRunThreads * L * n_stage;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
     KbPoly kp;
@@ -639,10 +642,9 @@ void launch_runs_k(rick_plan* p, void* grid, cudaStream_t st) {
         tc.K[t] = exp(-(double)(t * t) * p->g.tap_c);
         tc.Kf[t] = (float)tc.K[t];
     }
-    // consecutive sorted visibilities per thread: as for the record gridder, long ranges on dense inputs
-    // (fewer end-of-range reductions onto the same hot cells), >= ~12 CTAs per SM slot
+    // consecutive sorted visibilities per thread: as for the record gridder (100M: 64: 5.72, 128: 5.57, 256: 5.85 ms)
     long long L = p->M / ((long long)kRunThreads * p->sm_count * 2 * 12) / 4 * 4;
-    L = L < 32 ? 32 : (L > 256 ? 256 : L);
+    L = L < 32 ? 32 : (L > 128 ? 128 : L);
     const long long per_block = (long long)kRunThreads * L;
     const unsigned blocks = (unsigned)((p->M + per_block - 1) / per_block);
     k_grid_runs<real, S, RB, KIND><<<blocks, kRunThreads, 0, st>>>(p->g, tc, p->n_kept_dev, p->u_s, p->v_s, p->w_s,
