@@ -16,10 +16,17 @@
 namespace {
 
 constexpr int kRadix = 1 << RICK_RADIX_BITS_MAX;   // 512 digit values at most
-constexpr int kSortThreads = 256;
-constexpr int kSortItems = 32;
-constexpr int kSortTile = kSortThreads * kSortItems;   // 8192 keys per tile
-constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortTile = 8192;                        // keys per tile
+// shape of a one-sweep CTA: 256 threads x 32 keys, or, for the plain passes over 9-bit digits, 512 threads x 16 keys
+// (one digit per thread, 64 registers, two CTAs = 32 warps per SM: 0.269 -> 0.228 ms for the three passes of config 10M;
+// the same shape on 8-bit digits, where half the threads would own no digit, measured slower: 22.2 against 19.6 ms on
+// hotspot, and 54 against 46 ms for the gather variant at one CTA per SM)
+template <int kBits, bool kGather> struct SortShape {
+    static constexpr int kThreads = (kBits == 9 && !kGather) ? 512 : 256;
+    static constexpr int kItems = kSortTile / kThreads;
+    static constexpr int kWarps = kThreads / 32;
+    static constexpr int kMinBlocks = kThreads == 512 ? 2 : ((kBits == 8 && !kGather) ? 3 : 2);
+};
 constexpr int kSortAhead = 48;     // tickets between a tile and the one whose input it sends on its way to the L2
 
 struct SortLayout {
@@ -209,8 +216,9 @@ __device__ __forceinline__ void gather_one(const GatherOut& o, size_t src, size_
     o.gc[pos] = make_float2(ws * a.w, ws * b.x);
 }
 
-// sized by the digit width: 74 KB for 8-bit digits (three CTAs per SM), 84 KB for 9-bit digits (two)
-template <int kBits> struct SortSmem {
+// sized by the digit width and the CTA shape: 74 KB for 8-bit digits (256 threads, three CTAs per SM), 84 KB for the
+// gather passes over 9-bit digits (256 threads, two CTAs), 100 KB for the plain ones (512 threads, two CTAs)
+template <int kBits, int kSortWarps> struct SortSmem {
     uint32_t warp_cnt[kSortWarps][1 << kBits];   // per-warp digit counts -> exclusive offsets over warps
     uint32_t tile_excl[1 << kBits];              // first slot of each digit in the exchanged tile
     uint32_t glob[1 << kBits];                   // global position of slot i of digit d = glob[d] + i
@@ -220,6 +228,10 @@ template <int kBits> struct SortSmem {
     uint32_t tile;
 };
 
+template <int kBits, bool kGather> constexpr int sort_smem_bytes() {
+    return (int)sizeof(SortSmem<kBits, SortShape<kBits, kGather>::kWarps>);
+}
+
 // kGather: this is the last pass and nobody asked for the sorted (key, index) arrays: instead of writing them,
 // the tile gathers its visibilities straight to their final positions (the gather's random reads hide
 // under the pass's arithmetic, and 12 bytes per visibility of key/index traffic disappear).
@@ -228,7 +240,7 @@ template <int kBits> struct SortSmem {
 // hotspot; the gather variant keeps two CTAs of 128 registers, it needs them for the fp64 coordinates); the keys go to their exchange slots before the look-back, and the input indices are
 // loaded only then, in flight during the look-back, and follow into the slots the ranks (now slot numbers) name.
 template <bool kFirst, int kBits, bool kGather>
-__global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2) k_onesweep(const uint32_t* __restrict__ key_in,
+__global__ void __launch_bounds__((SortShape<kBits, kGather>::kThreads), (SortShape<kBits, kGather>::kMinBlocks)) k_onesweep(const uint32_t* __restrict__ key_in,
                                                                const uint32_t* __restrict__ idx_in,
                                                                uint32_t* __restrict__ key_out,
                                                                uint32_t* __restrict__ idx_out, long long M, int shift,
@@ -237,7 +249,10 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
                                                                uint32_t* __restrict__ ticket, uint32_t epoch,
                                                                GatherOut go, uint32_t ahead) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem<kBits>& sm = *reinterpret_cast<SortSmem<kBits>*>(smem_raw);
+    typedef SortShape<kBits, kGather> Shape;
+    constexpr int kSortThreads = Shape::kThreads, kSortItems = Shape::kItems, kSortWarps = Shape::kWarps;
+    typedef SortSmem<kBits, kSortWarps> Smem;
+    Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < kSortWarps * (1 << kBits); i += kSortThreads) (&sm.warp_cnt[0][0])[i] = 0;
@@ -262,7 +277,8 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
     static_assert(kDigitsPerThread >= 1, "digit width too small for the block size");
 
     uint32_t k[kSortItems];
-    uint16_t rank[kSortItems];              // rank in the warp's digit bucket, later the exchange slot (< 8192)
+    typedef typename std::conditional<(kSortItems <= 16), uint32_t, uint16_t>::type rank_t;
+    rank_t rank[kSortItems];                // rank in the warp's digit bucket, later the exchange slot (< 8192)
     const unsigned lt = (1u << lane) - 1u;
     const bool full = tile_base + kSortTile <= M;     // every tile but the last: no validity tests
     // rank of an item among the items of its warp with the same digit (stable: lanes in order), by one
@@ -298,7 +314,7 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
                 sm.warp_cnt[warp][d] = c + (uint32_t)__popc(peers);
             }
             c = __shfl_sync(0xffffffffu, c, valid ? leader : lane);
-            rank[j] = (uint16_t)(c + (uint32_t)__popc(peers & lt));
+            rank[j] = (rank_t)(c + (uint32_t)__popc(peers & lt));
             __syncwarp();
         }
     };
@@ -362,7 +378,7 @@ __global__ void __launch_bounds__(kSortThreads, (kBits == 8 && !kGather) ? 3 : 2
             const uint32_t d = (k[j] >> shift) & mask;
             const uint32_t lp = sm.tile_excl[d] + sm.warp_cnt[warp][d] + rank[j];
             sm.xkey[lp] = k[j];
-            rank[j] = (uint16_t)lp;
+            rank[j] = (rank_t)lp;
         }
     }
     // the input indices, in flight during the look-back
@@ -477,16 +493,15 @@ size_t rick_bin_workspace_bytes(const rick_plan* p, long long M) {
 }
 
 int rick_bin_init() {
-    const int b8 = (int)sizeof(SortSmem<8>), b9 = (int)sizeof(SortSmem<9>);
     const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
-    if (cudaFuncSetAttribute(k_onesweep<true, 8, false>, a, b8) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 9, false>, a, b9) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 8, false>, a, b8) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 9, false>, a, b9) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 8, true>, a, b8) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<true, 9, true>, a, b9) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 8, true>, a, b8) != cudaSuccess ||
-        cudaFuncSetAttribute(k_onesweep<false, 9, true>, a, b9) != cudaSuccess)
+    if (cudaFuncSetAttribute(k_onesweep<true, 8, false>, a, sort_smem_bytes<8, false>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, false>, a, sort_smem_bytes<9, false>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, false>, a, sort_smem_bytes<8, false>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, false>, a, sort_smem_bytes<9, false>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 8, true>, a, sort_smem_bytes<8, true>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<true, 9, true>, a, sort_smem_bytes<9, true>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 8, true>, a, sort_smem_bytes<8, true>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_onesweep<false, 9, true>, a, sort_smem_bytes<9, true>()) != cudaSuccess)
         return RICK_ECUDA;
     return RICK_OK;
 }
@@ -553,7 +568,11 @@ int rick_bin_impl(rick_plan* p, long long M, const float* u, const float* v, con
                                       : (nine ? k_onesweep<false, 9, true> : k_onesweep<false, 8, true>))
                              : (first ? (nine ? k_onesweep<true, 9, false> : k_onesweep<true, 8, false>)
                                       : (nine ? k_onesweep<false, 9, false> : k_onesweep<false, 8, false>));
-            kern<<<n_tiles, kSortThreads, nine ? sizeof(SortSmem<9>) : sizeof(SortSmem<8>), st>>>(kin, iin, kout, iout, M, lay.shift[pass],
+            const int threads = gath ? (nine ? SortShape<9, true>::kThreads : SortShape<8, true>::kThreads)
+                                     : (nine ? SortShape<9, false>::kThreads : SortShape<8, false>::kThreads);
+            const int smem = gath ? (nine ? sort_smem_bytes<9, true>() : sort_smem_bytes<8, true>())
+                                  : (nine ? sort_smem_bytes<9, false>() : sort_smem_bytes<8, false>());
+            kern<<<n_tiles, threads, smem, st>>>(kin, iin, kout, iout, M, lay.shift[pass],
                                                                  ws.hist + pass * kRadix, ws.status, ws.ticket + pass,
                                                                  (uint32_t)(pass + 1), go,
                                                                  (uint32_t)kSortAhead);
