@@ -201,8 +201,10 @@ template <typename C2, int L> struct ColB {
     static constexpr int kIssuers = L < T ? L : T;                // threads that issue row copies
     static constexpr int kRowsPerIssuer = L / kIssuers;
     static constexpr size_t smem = 2 * sizeof(C2) * L * C + sizeof(C2) * L + 2 * sizeof(unsigned long long);
-    // resident CTAs the register allocation must leave room for (two of 256 threads: <= 128 registers)
-    static constexpr int kMinBlocks = (sizeof(C2) == 16 && L == 128) ? 1 : (T >= 256 ? 2 : 3);
+    // resident CTAs the register allocation must leave room for: three (of 256 threads: 80 registers, the fp64 sums
+    // and n - 1 values partly in local memory, but 24 instead of 16 warps per SM: hotspot 9.45 -> 9.15 ms, 500M 4.39 ->
+    // 4.36 ms; shared memory, 66 KB per CTA at N2 = 128, allows no more); the 128-row fp64 tile fits once
+    static constexpr int kMinBlocks = (sizeof(C2) == 16 && L == 128) ? 1 : 3;
 };
 
 template <typename C2, int N1, int N2>
