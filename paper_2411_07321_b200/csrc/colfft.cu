@@ -190,9 +190,10 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         // the fraction, two's complement, in the low 23 mantissa bits (|w_k nm1| < 2^28 turns).
         const double z = fma(wk, nm1r[e], 805306368.0);
         const float gq = __int_as_float(0x3F800000 | (__double2loint(z) & 0x007FFFFF));   // 1 + fraction
-        const float t = gq - 1.5f;                             // fraction - 1/2 in [-1/2, 1/2) turns, exact
+        // 2 pi (fraction - 1/2), in [-pi, pi): one FFMA (rounding: 2^-24 pi rad, below the 2^-23-turn phase step)
+        const float t = fmaf(gq, 6.283185307179586f, -9.42477796076938f);
         float sn, cs;
-        __sincosf(6.283185307179586f * t, &sn, &cs);           // MUFU on [-pi, pi]: abs error < 5e-7
+        __sincosf(t, &sn, &cs);                                // MUFU on [-pi, pi]: abs error < 5e-7
         acc[e] += (double)(sn * v.y - cs * v.x);               // the half turn negates sine and cosine
     };
 

@@ -165,9 +165,10 @@ template <int E> struct Screen<float, E> {
     RICK_DI double term(int e, float2 v, double wk) {
         const double z = fma(wk, nm1[e], 805306368.0);                     // 1.5 * 2^29: fraction in the low 23 bits
         const float gq = __int_as_float(0x3F800000 | (__double2loint(z) & 0x007FFFFF));
-        const float t = gq - 1.5f;                                         // fraction - 1/2 in [-1/2, 1/2) turns, exact
+        // 2 pi (fraction - 1/2), in [-pi, pi): one FFMA (rounding: 2^-24 pi rad, below the 2^-23-turn phase step)
+        const float t = fmaf(gq, 6.283185307179586f, -9.42477796076938f);
         float sn, cs;
-        __sincosf(6.283185307179586f * t, &sn, &cs);
+        __sincosf(t, &sn, &cs);
         return (double)(sn * v.y - cs * v.x);                              // the half turn negates sine and cosine
     }
     RICK_DI void next(int) {}
