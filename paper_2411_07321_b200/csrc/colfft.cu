@@ -189,7 +189,9 @@ __global__ void __launch_bounds__(kT, 1) k_colfft_wcorrect(RickGeom g, const flo
         // made the screen XU-bound): adding 1.5 * 2^29 rounds the product (one DFMA) to 2^-23 turns and leaves
         // the fraction, two's complement, in the low 23 mantissa bits (|w_k nm1| < 2^28 turns).
         const double z = fma(wk, nm1r[e], 805306368.0);
-        const float gq = __int_as_float(0x3F800000 | (__double2loint(z) & 0x007FFFFF));   // 1 + fraction
+        uint32_t gbits;                                                     // 1 + fraction: (lo & mantissa) | one, one LOP3
+        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(gbits) : "r"((uint32_t)__double2loint(z)), "r"(0x007FFFFFu), "r"(0x3F800000u));
+        const float gq = __uint_as_float(gbits);   // 1 + fraction
         // 2 pi (fraction - 1/2), in [-pi, pi): one FFMA (rounding: 2^-24 pi rad, below the 2^-23-turn phase step)
         const float t = fmaf(gq, 6.283185307179586f, -9.42477796076938f);
         float sn, cs;

@@ -164,7 +164,9 @@ template <int E> struct Screen<float, E> {
     RICK_DI void init(int e, double nm1v, const RickGeom&) { nm1[e] = nm1v; }
     RICK_DI double term(int e, float2 v, double wk) {
         const double z = fma(wk, nm1[e], 805306368.0);                     // 1.5 * 2^29: fraction in the low 23 bits
-        const float gq = __int_as_float(0x3F800000 | (__double2loint(z) & 0x007FFFFF));
+        uint32_t gbits;                                                     // 1 + fraction: (lo & mantissa) | one, one LOP3
+        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(gbits) : "r"((uint32_t)__double2loint(z)), "r"(0x007FFFFFu), "r"(0x3F800000u));
+        const float gq = __uint_as_float(gbits);
         // 2 pi (fraction - 1/2), in [-pi, pi): one FFMA (rounding: 2^-24 pi rad, below the 2^-23-turn phase step)
         const float t = fmaf(gq, 6.283185307179586f, -9.42477796076938f);
         float sn, cs;
